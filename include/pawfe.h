@@ -1,0 +1,170 @@
+/*
+ * pawfe.h -- C ABI of libpawfe.so: the R-ChFSI filter hot path of PAW-FE (arxiv/paper_2604_26037)
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are lines of the paper text with the section / equation / algorithm they
+ * fall in.  The library computes, with its own CUDA kernels only (there is no CPU fallback):
+ *
+ *   H = H_loc + sum_a C^a D^a C^a^dagger,   S = M + sum_a C^a dS^a C^a^dagger      (Eq. 13, 16; L125-L138)
+ *   S^-1approx = M_D^-1 - sum_a M_D^-1 C^a Delta^a_Sinv C^a^dagger M_D^-1           (Eq. 28-29; L219-L228)
+ *   Algorithm 2: residual-based Chebyshev filter of degree m on [bW, bU]          (L250-L282)
+ *
+ * on a uniform hexahedral spectral-element mesh (tensor-product GLL Lagrange basis of order p,
+ * L116, L307) through the cell-matrix strategy of section 4.3 (L337-L347): gather to cells, dense
+ * cell-matrix x cell-vector-block contraction, scatter-add assembly, plus atom-local projector
+ * contractions for the non-local PAW terms.
+ *
+ * Conventions
+ *  - Every function returns a pawfe_status and never throws across the ABI; pawfe_last_error()
+ *    gives the text of the last failure on that context.
+ *  - "host" / "device" is stated for every pointer.  Device pointers must belong to the context's
+ *    device.  All work is enqueued on the context's CUDA stream; hot calls (apply_*, cheb_filter,
+ *    col_norms, axpy helpers) allocate nothing and do not synchronise the host, except where stated.
+ *  - The library OWNS the operators (cell matrices, projector blocks, couplings, lumped mass) and
+ *    frees them in pawfe_destroy.  The CALLER owns all vector blocks and the filter workspace.
+ *  - Vector blocks are row-major [dof][vec] ("vec" contiguous), leading dimension ld in ELEMENTS.
+ *    Real contexts: element = double (PAWFE_FP64) or float (PAWFE_FP32 / PAWFE_TF32).
+ *    Complex contexts (k-point given): element = interleaved (re, im) pair of that type.
+ *  - Node numbering is lexicographic over the stored node grid: J = (ix*Ny + iy)*Nz + iz, with
+ *    i = c*p + a for cell c and local GLL index a.  Periodic: N_d = ncells_d*p.  Dirichlet:
+ *    N_d = ncells_d*p + 1 nodes are STORED, boundary rows are ignored on input and written as 0.
+ *  - A device that is not compute capability 10.x gives PAWFE_EUNSUPPORTED.
+ */
+#ifndef PAWFE_H
+#define PAWFE_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pawfe_ctx pawfe_ctx; /* opaque, owned by the library */
+
+typedef enum {
+  PAWFE_OK = 0,
+  PAWFE_EINVAL = 1,       /* bad argument */
+  PAWFE_ENOMEM = 2,       /* device or host allocation failed */
+  PAWFE_ECUDA = 3,        /* a CUDA call or kernel failed; see pawfe_last_error */
+  PAWFE_ESTATE = 4,       /* call made before the data it needs exists */
+  PAWFE_EUNSUPPORTED = 5  /* not an sm_100 device, or an unsupported (p, B, precision) */
+} pawfe_status;
+
+/* Arithmetic of the cell contraction (section 4.4; L11, L27 for TF32):
+ *   FP64: every step in double (reference mode).
+ *   FP32: FP32 storage and arithmetic inside H S^-1approx.
+ *   TF32: FP32 storage; operands of the cell contraction rounded to TF32 inside tcgen05 tensor
+ *         cores, FP32 accumulation.  Nothing else is TF32. */
+typedef enum { PAWFE_FP64 = 0, PAWFE_FP32 = 1, PAWFE_TF32 = 2 } pawfe_prec;
+typedef enum { PAWFE_PERIODIC = 0, PAWFE_DIRICHLET = 1 } pawfe_bc;
+
+/* ---- lifetime ------------------------------------------------------------------------------ */
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the legacy
+ * default stream); the caller keeps ownership of the stream. */
+pawfe_status pawfe_create(pawfe_ctx** out, int device, void* cuda_stream);
+pawfe_status pawfe_destroy(pawfe_ctx* ctx);
+/* Text of the last error on this context ("" if none).  Valid until the next call on ctx. */
+const char* pawfe_last_error(const pawfe_ctx* ctx);
+/* Change the stream later calls are enqueued on. */
+pawfe_status pawfe_set_stream(pawfe_ctx* ctx, void* cuda_stream);
+
+/* ---- mesh and cell operators (Eq. 12-13; Eq. 31-33; M_D of L228) -------- */
+
+/* Uniform mesh of box[0] x box[1] x box[2] bohr with ncells[d] cells per direction, FE order p
+ * (2 <= p <= 7; p+1 GLL nodes per direction per cell).  kpt: host, 3 doubles (Bloch vector in
+ * 1/bohr) or NULL for a real (Gamma, no phase) context.  Periodic meshes need an even ncells[d].
+ * Builds the 1-D GLL / Gauss-Legendre tables, the reference cell matrices and the lumped mass. */
+pawfe_status pawfe_mesh_create(pawfe_ctx* ctx, const int ncells[3], const double box[3], int p,
+                               pawfe_bc bc, const double* kpt);
+
+/* Local potential V(x) = - sum_a sum_images Z_a exp(-|x - R_a - L|^2 / (2 sigma_a^2)); periodic:
+ * the 27 nearest images; Dirichlet: none (stands in for V_eff + V_z of Eq. 2).
+ * pos: host, 3*natoms doubles; Z, sigma: host, natoms doubles.
+ * Builds on the device, in FP64 arithmetic, every cell matrix
+ *   H^e = 1/2 K^e + V^e + 1/2 |k|^2 M^e - i sum_d k_d G_d^e                (Eq. 13 / Eq. 32)
+ * with V^e on a (p+2)^3 Gauss-Legendre grid, and stores it as FP32 (always) and FP64 (if
+ * keep_fp64 != 0; needed by PAWFE_FP64 applies and by the residual set-up of the filter).
+ * Synchronises the host. */
+pawfe_status pawfe_local_potential_gaussians(pawfe_ctx* ctx, int natoms, const double* pos,
+                                             const double* Z, const double* sigma, int keep_fp64);
+
+/* ---- atoms and projectors (Eq. 16-17; Eq. 34; Eq. 28-29) ----------- */
+
+/* One species: nproj projectors p_alpha(d) = amp * r^l exp(-r^2 / 2 sigma^2) (1-(r/rc)^2)^2 Y_lm(d/r)
+ * for r < rc (real orthonormal Y_lm, l <= 2), 0 otherwise.  proj_l, proj_m: host, nproj ints;
+ * proj_sigma, proj_amp: host, nproj doubles.  pos: host, 3*natoms doubles.
+ * D (= Delta_H) and dS (= Delta_S): host, natoms*nproj*nproj doubles, real symmetric per atom.
+ * Builds the cell-level projector blocks C^{e,a} (Eq. 34) on a (2(p+2))^3 Gauss-Legendre grid for
+ * every (cell, atom) pair whose cell meets the atom's sphere (minimum image when periodic; phase
+ * e^{ik.(R_a + d)} when complex), G^a = C^a^dagger M_D^-1 C^a and
+ * Delta^a_Sinv = (I + dS^a G^a)^-1 dS^a (Eq. 29).  Needs rc < min(box)/2 when periodic.
+ * Synchronises the host. */
+pawfe_status pawfe_atoms_create(pawfe_ctx* ctx, int natoms, const double* pos, int nproj,
+                                const int* proj_l, const int* proj_m, const double* proj_sigma,
+                                const double* proj_amp, double rc, const double* D, const double* dS);
+
+/* Replace D (Delta_H changes every SCF step, Eq. 18).  host, natoms*nproj*nproj. */
+pawfe_status pawfe_update_coupling(pawfe_ctx* ctx, const double* D);
+
+/* ---- queries ------------------------------------------------------------------------------- */
+
+pawfe_status pawfe_num_dofs(const pawfe_ctx* ctx, long* M);          /* stored nodes */
+pawfe_status pawfe_num_pairs(const pawfe_ctx* ctx, long* npairs);    /* (cell, atom) pairs */
+/* Copy one FP64 cell matrix H^e (n x n, row-major, complex interleaved if k-point) to host memory.
+ * Needs keep_fp64.  For tests; synchronises. */
+pawfe_status pawfe_get_cell_matrix(pawfe_ctx* ctx, long cell, double* out_host);
+/* Copy Delta_Sinv (natoms*nproj*nproj, complex interleaved if k-point) to host.  For tests. */
+pawfe_status pawfe_get_sinv_coupling(pawfe_ctx* ctx, double* out_host);
+
+/* ---- operator applications on a block (section 4.3) ------------------------------ */
+
+/* Y = A X for A in {H, S, S^-1approx}.  X, Y: device, [dof][vec] with leading dimension ld >= B,
+ * element type given by prec (see Conventions); X and Y must not overlap.  1 <= B <= 512.
+ * Boundary (Dirichlet) rows of X are ignored, those of Y are written as 0. */
+pawfe_status pawfe_apply_H(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+pawfe_status pawfe_apply_S(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+pawfe_status pawfe_apply_Sinv(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+
+/* ---- Algorithm 2 (L250-L282) --------------------------------------------------------------- */
+
+/* Bytes of device workspace pawfe_cheb_filter needs for block width B (leading dimension B). */
+pawfe_status pawfe_filter_workspace(pawfe_ctx* ctx, pawfe_prec prec, int B, size_t* bytes);
+
+/* Residual-based Chebyshev filter of degree m >= 1:
+ *   step 1  e = (bU-bW)/2, c = (bU+bW)/2, zeta = e/(b0-c), gamma = 2/zeta                    (L257)
+ *   step 2  Y = H X - S X Lambda                      always FP64 arithmetic                  (L260, L374)
+ *   step 3  R_X = 0, R_Y = (zeta/e) Y, Lambda_X = 1, Lambda_Y = (zeta/e)(Lambda - c)           (L262-L264)
+ *   step 4  for theta = 2..m: zeta1 = 1/(gamma - zeta);
+ *             R_X <- (2 zeta1/e) H S^-1approx R_Y - (2 zeta1 c/e) R_Y - zeta zeta1 R_X  [prec]
+ *                    + (2 zeta1/e) Y Lambda_Y                                        [FP64 add, L374]
+ *             Lambda_X likewise; swap; zeta <- zeta1                                          (L269-L279)
+ *   step 5  X <- S^-1approx R_Y + X Lambda_Y                                                    (L282)
+ * X: device, in Psi_in / out Psi_f, [dof][vec], leading dimension ld, element type by prec.
+ * lambda: HOST, B doubles.  workspace: device, >= pawfe_filter_workspace bytes, 256-byte aligned.
+ * The B scalars are copied to the device asynchronously from an internal pinned buffer. */
+pawfe_status pawfe_cheb_filter(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW, double bU,
+                               void* X, const double* lambda, long ld, int B,
+                               void* workspace, size_t workspace_bytes);
+
+/* Same call with HOST vector block X_host (B columns, leading dimension ld): copies it to an
+ * internal device block, filters, copies Psi_f back, and synchronises.  The internal block and
+ * workspace are allocated on first use for the largest B seen. */
+pawfe_status pawfe_cheb_filter_host(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW,
+                                    double bU, void* X_host, const double* lambda, long ld, int B);
+
+/* Column 2-norms ||x_i||_2, i < B, accumulated in FP64 (L290).  X: device, element type by prec;
+ * out: DEVICE, B doubles. */
+pawfe_status pawfe_col_norms(pawfe_ctx* ctx, pawfe_prec prec, const void* X, long ld, int B, double* out);
+
+/* Count of kernels this context has launched so far (bench.py's gpu_launches). */
+pawfe_status pawfe_launch_count(const pawfe_ctx* ctx, long* n);
+
+/* Name of the cell-contraction kernel variant a given (prec, B) runs ("tcgen05_tf32", "simt_fp32",
+ * "simt_fp64", ...).  Static string. */
+const char* pawfe_cell_kernel_name(const pawfe_ctx* ctx, pawfe_prec prec, int B);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAWFE_H */
