@@ -38,6 +38,9 @@
 #ifdef __cplusplus
 extern "C" {
 #endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default) /* the library is built with -fvisibility=hidden */
+#endif
 
 typedef struct pawfe_ctx pawfe_ctx; /* opaque, owned by the library */
 
@@ -164,6 +167,9 @@ pawfe_status pawfe_launch_count(const pawfe_ctx* ctx, long* n);
  * "simt_fp64", ...).  Static string. */
 const char* pawfe_cell_kernel_name(const pawfe_ctx* ctx, pawfe_prec prec, int B);
 
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,201 @@
+// api_apply.cu -- operator applications A X, A in {H, S, S^-1approx} (section 4.3; Eq. 28)
+// as sequences of kernel launches on the context's stream.  No allocation, no host synchronisation
+// (except growing the projection scratch the first time a wider block is seen).
+#include "common.h"
+#include "host_util.h"
+#include "kernels_simt.cuh"
+#include "kernels_stream.cuh"
+#include "api_internal.h"
+#include "apply_impl.h"
+#include <algorithm>
+
+namespace {
+
+template <typename TC> struct OpData;
+template <> struct OpData<double> {
+  static const double* H(const pawfe_ctx* c) { return (const double*)c->d_H64; }
+  static const double* Mref(const pawfe_ctx* c) { return c->d_Mref64; }
+  static int lda(const pawfe_ctx* c) { return c->n; }
+  static const double* Cd(const pawfe_ctx* c) { return (const double*)c->d_Cd64; }
+  static const double* D(const pawfe_ctx* c) { return (const double*)c->d_D64; }
+  static const double* dS(const pawfe_ctx* c) { return (const double*)c->d_dS64; }
+  static const double* dSinv(const pawfe_ctx* c) { return (const double*)c->d_dSinv64; }
+};
+template <> struct OpData<double2> {
+  static const double2* H(const pawfe_ctx* c) { return (const double2*)c->d_H64; }
+  static const double2* Mref(const pawfe_ctx* c) { return (const double2*)c->d_Mref64; }
+  static int lda(const pawfe_ctx* c) { return c->n; }
+  static const double2* Cd(const pawfe_ctx* c) { return (const double2*)c->d_Cd64; }
+  static const double2* D(const pawfe_ctx* c) { return (const double2*)c->d_D64; }
+  static const double2* dS(const pawfe_ctx* c) { return (const double2*)c->d_dS64; }
+  static const double2* dSinv(const pawfe_ctx* c) { return (const double2*)c->d_dSinv64; }
+};
+template <> struct OpData<float> {
+  static const float* H(const pawfe_ctx* c) { return (const float*)c->d_H32; }
+  static const float* Mref(const pawfe_ctx* c) { return c->d_Mref32; }
+  static int lda(const pawfe_ctx* c) { return c->ldk; }
+  static const float* Cd(const pawfe_ctx* c) { return (const float*)c->d_Cd32; }
+  static const float* D(const pawfe_ctx* c) { return (const float*)c->d_D32; }
+  static const float* dS(const pawfe_ctx* c) { return (const float*)c->d_dS32; }
+  static const float* dSinv(const pawfe_ctx* c) { return (const float*)c->d_dSinv32; }
+};
+template <> struct OpData<float2> {
+  static const float2* H(const pawfe_ctx* c) { return (const float2*)c->d_H32; }
+  static const float2* Mref(const pawfe_ctx* c) { return (const float2*)c->d_Mref32; }
+  static int lda(const pawfe_ctx* c) { return c->ldk; }
+  static const float2* Cd(const pawfe_ctx* c) { return (const float2*)c->d_Cd32; }
+  static const float2* D(const pawfe_ctx* c) { return (const float2*)c->d_D32; }
+  static const float2* dS(const pawfe_ctx* c) { return (const float2*)c->d_dS32; }
+  static const float2* dSinv(const pawfe_ctx* c) { return (const float2*)c->d_dSinv32; }
+};
+
+template <typename TY>
+pawfe_status zero_block(pawfe_ctx* c, TY* Y, long ldy, int B) {
+  if (ldy == B) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * B * sizeof(TY), c->stream));
+  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(TY), 0, (size_t)B * sizeof(TY), c->M, c->stream));
+  return PAWFE_OK;
+}
+
+template <typename TX, typename TY, typename TC, bool TF32>
+pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, const TX* X, long ldx, TY* Y,
+                         long ldy, int B, int in_scale, double alpha) {
+  constexpr int BV = (sizeof(TC) == 16) ? 16 : 32;
+  size_t smem = (size_t)c->n * 16 + (size_t)c->n * BV * sizeof(TC);
+  auto kern = k_cell_simt<TX, TY, TC, BV, TF32>;
+  CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<dim3(c->ncell, ceil_div(B, BV)), 256, smem, c->stream>>>(c->md, A, cell_stride, lda, X, ldx, Y, ldy, B,
+                                                                  in_scale, alpha);
+  KERNEL_CHECK(c, "k_cell_simt");
+  return PAWFE_OK;
+}
+
+}  // namespace
+
+// Y (+)= nonlocal part:  Y += out_scale o C (scale * Delta (C^dagger (in_scale o X)))
+template <typename TX, typename TY, typename TC>
+pawfe_status pawfe_apply_nonlocal(pawfe_ctx* c, const TC* Delta, double scale, const TX* X, long ldx, int in_scale,
+                                  TY* Y, long ldy, int out_scale, int B) {
+  if (c->npairs == 0) return PAWFE_OK;
+  TRY(pawfe_ensure_P(c, B));
+  TC* P = (TC*)c->d_P;
+  TC* W = P + (size_t)c->natoms * c->npj * B;
+  size_t smem = (size_t)c->n * 16 + 4 * PAWFE_MAX_NPJ * 32 * sizeof(TC);
+  k_proj<TX, TC><<<dim3(c->natoms, ceil_div(B, 32)), 128, smem, c->stream>>>(
+      c->md, 0, c->d_atom_pair_start, c->d_pair_cell, OpData<TC>::Cd(c), c->npj, X, ldx, B, in_scale, P, B);
+  KERNEL_CHECK(c, "k_proj");
+  k_coupling<TC><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(Delta, c->npj, P, B, B, scale, W);
+  KERNEL_CHECK(c, "k_coupling");
+  k_nl_scatter<TY, TC><<<dim3((unsigned)c->npairs, ceil_div(B, 32)), 128, 0, c->stream>>>(
+      c->md, 0, c->d_pair_cell, c->d_pair_atom, OpData<TC>::Cd(c), c->npj, W, B, B, out_scale, Y, ldy);
+  KERNEL_CHECK(c, "k_nl_scatter");
+  return PAWFE_OK;
+}
+
+// Y = H X (op 0) or S X (op 1)
+template <typename TX, typename TY, typename TC>
+pawfe_status pawfe_apply_HS(pawfe_ctx* c, int op, bool tf32, const TX* X, long ldx, TY* Y, long ldy, int B) {
+  TRY(zero_block(c, Y, ldy, B));
+  const TC* A = op == 0 ? OpData<TC>::H(c) : OpData<TC>::Mref(c);
+  long stride = op == 0 ? (long)c->n * OpData<TC>::lda(c) : 0;
+  if (tf32 && op == 0) TRY((launch_cell<TX, TY, TC, true>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0)));
+  else TRY((launch_cell<TX, TY, TC, false>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0)));
+  const TC* Delta = op == 0 ? OpData<TC>::D(c) : OpData<TC>::dS(c);
+  return pawfe_apply_nonlocal<TX, TY, TC>(c, Delta, 1.0, X, ldx, 0, Y, ldy, 0, B);
+}
+
+// Y = S^-1approx X = M_D^-1 X - M_D^-1 C Delta_Sinv C^dagger M_D^-1 X   (Eq. 28)
+template <typename TX, typename TY, typename TC>
+pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, long ldy, int B) {
+  typedef typename ScalarTraits<TX>::real RX;
+  typedef typename ScalarTraits<TY>::real RY;
+  const int cw = ScalarTraits<TX>::cplx ? 2 : 1;
+  k_scale_mdinv<RX, RY><<<4 * c->sm_count, 256, 0, c->stream>>>(c->md, (const RX*)X, ldx * cw, (RY*)Y, ldy * cw, B * cw);
+  KERNEL_CHECK(c, "k_scale_mdinv");
+  return pawfe_apply_nonlocal<TX, TY, TC>(c, OpData<TC>::dSinv(c), -1.0, X, ldx, 1, Y, ldy, 1, B);
+}
+
+// explicit instantiations used by the other translation units
+#define INST(TX, TY, TC)                                                                                          \
+  template pawfe_status pawfe_apply_HS<TX, TY, TC>(pawfe_ctx*, int, bool, const TX*, long, TY*, long, int);       \
+  template pawfe_status pawfe_apply_Sinv_impl<TX, TY, TC>(pawfe_ctx*, const TX*, long, TY*, long, int);
+INST(double, double, double)
+INST(float, double, double)
+INST(float, float, float)
+INST(double2, double2, double2)
+INST(float2, double2, double2)
+INST(float2, float2, float2)
+#undef INST
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+static pawfe_status check_apply(pawfe_ctx* c, pawfe_prec prec, const void* X, void* Y, long ld, int B, bool need_pot) {
+  if (!c || !X || !Y || B < 1 || B > 512 || ld < B) { if (c) c->err = "bad block arguments"; return PAWFE_EINVAL; }
+  if (prec != PAWFE_FP64 && prec != PAWFE_FP32 && prec != PAWFE_TF32) return PAWFE_EINVAL;
+  if (!c->have_mesh || !c->have_atoms || (need_pot && !c->have_pot)) { c->err = "operators not set up"; return PAWFE_ESTATE; }
+  if (need_pot && prec == PAWFE_FP64 && !c->have_h64) { c->err = "FP64 cell matrices were not kept (keep_fp64 = 0)"; return PAWFE_ESTATE; }
+  cudaError_t e = cudaSetDevice(c->device);
+  if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return PAWFE_ECUDA; }
+  return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_apply_H(pawfe_ctx* c, pawfe_prec prec, const void* X, void* Y, long ld, int B) {
+  TRY(check_apply(c, prec, X, Y, ld, B, true));
+  return pawfe_apply_H_any(c, prec, X, ld, Y, ld, B);
+}
+extern "C" pawfe_status pawfe_apply_S(pawfe_ctx* c, pawfe_prec prec, const void* X, void* Y, long ld, int B) {
+  TRY(check_apply(c, prec, X, Y, ld, B, false));
+  bool f64 = prec == PAWFE_FP64;
+  if (c->cplx) return f64 ? pawfe_apply_HS<double2, double2, double2>(c, 1, false, (const double2*)X, ld, (double2*)Y, ld, B)
+                          : pawfe_apply_HS<float2, float2, float2>(c, 1, false, (const float2*)X, ld, (float2*)Y, ld, B);
+  return f64 ? pawfe_apply_HS<double, double, double>(c, 1, false, (const double*)X, ld, (double*)Y, ld, B)
+             : pawfe_apply_HS<float, float, float>(c, 1, false, (const float*)X, ld, (float*)Y, ld, B);
+}
+extern "C" pawfe_status pawfe_apply_Sinv(pawfe_ctx* c, pawfe_prec prec, const void* X, void* Y, long ld, int B) {
+  TRY(check_apply(c, prec, X, Y, ld, B, false));
+  bool f64 = prec == PAWFE_FP64;
+  if (c->cplx) return f64 ? pawfe_apply_Sinv_impl<double2, double2, double2>(c, (const double2*)X, ld, (double2*)Y, ld, B)
+                          : pawfe_apply_Sinv_impl<float2, float2, float2>(c, (const float2*)X, ld, (float2*)Y, ld, B);
+  return f64 ? pawfe_apply_Sinv_impl<double, double, double>(c, (const double*)X, ld, (double*)Y, ld, B)
+             : pawfe_apply_Sinv_impl<float, float, float>(c, (const float*)X, ld, (float*)Y, ld, B);
+}
+
+// H apply in the storage type of `prec`; the TF32 mode of a real context runs the tcgen05 kernel when it
+// supports the shape, otherwise the SIMT kernel with TF32-rounded operands.
+pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, long ldx, void* Y, long ldy, int B) {
+  if (prec == PAWFE_FP64) {
+    if (c->cplx) return pawfe_apply_HS<double2, double2, double2>(c, 0, false, (const double2*)X, ldx, (double2*)Y, ldy, B);
+    return pawfe_apply_HS<double, double, double>(c, 0, false, (const double*)X, ldx, (double*)Y, ldy, B);
+  }
+  bool tf32 = prec == PAWFE_TF32;
+  if (c->cplx) return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
+  if (tf32 && tc_supported(c, B)) {
+    TRY(zero_block(c, (float*)Y, ldy, B));
+    TRY(tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f));
+    return pawfe_apply_nonlocal<float, float, float>(c, OpData<float>::D(c), 1.0, (const float*)X, ldx, 0, (float*)Y, ldy, 0, B);
+  }
+  return pawfe_apply_HS<float, float, float>(c, 0, tf32, (const float*)X, ldx, (float*)Y, ldy, B);
+}
+
+extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec prec, int B) {
+  if (!c) return "none";
+  if (prec == PAWFE_FP64) return "simt_fp64";
+  if (prec == PAWFE_FP32) return "simt_fp32";
+  if (!c->cplx && tc_supported(c, B)) return "tcgen05_tf32";
+  return "simt_tf32_emulated";
+}
+
+extern "C" pawfe_status pawfe_col_norms(pawfe_ctx* c, pawfe_prec prec, const void* X, long ld, int B, double* out) {
+  if (!c || !X || !out || B < 1 || ld < B) return PAWFE_EINVAL;
+  if (!c->have_mesh) return PAWFE_ESTATE;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  CUDA_TRY(c, cudaMemsetAsync(out, 0, B * sizeof(double), c->stream));
+  const int cw = c->cplx ? 2 : 1;
+  dim3 grid(ceil_div(B, 32), std::min<long>(4 * c->sm_count, (c->M + 7) / 8)), block(32, 8);
+  if (prec == PAWFE_FP64) k_col_sumsq<double><<<grid, block, 0, c->stream>>>(c->M, B, cw, (const double*)X, ld, out);
+  else k_col_sumsq<float><<<grid, block, 0, c->stream>>>(c->M, B, cw, (const float*)X, ld, out);
+  KERNEL_CHECK(c, "k_col_sumsq");
+  k_sqrt_inplace<<<ceil_div(B, 128), 128, 0, c->stream>>>(out, B);
+  KERNEL_CHECK(c, "k_sqrt_inplace");
+  return PAWFE_OK;
+}

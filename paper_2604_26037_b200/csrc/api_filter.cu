@@ -1,0 +1,181 @@
+// api_filter.cu -- Algorithm 2 of the paper: the residual-based Chebyshev filter,
+// orchestrated on the host as a stream of kernel launches.  Mixed precision as in section 4.4 (L374):
+// residual set-up and the residual-source term in FP64, the bracket and H S^-1approx in the mode's precision.
+#include "common.h"
+#include "host_util.h"
+#include "kernels_stream.cuh"
+#include "api_internal.h"
+#include "apply_impl.h"
+#include <algorithm>
+#include <cstring>
+
+namespace {
+
+inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+struct WsLayout {
+  size_t y64, sx_t, ht, rx, ry, total;
+};
+
+// storage bytes per scalar: ss (4/8 real, 8/16 complex); FP64 scalar bytes: sd
+WsLayout ws_layout(long M, int B, size_t ss, size_t sd) {
+  WsLayout w;
+  size_t blk_s = align256((size_t)M * B * ss), blk_d = align256((size_t)M * B * sd);
+  if (2 * ss <= sd) blk_d = std::max(blk_d, 2 * blk_s);
+  w.y64 = 0;
+  w.sx_t = blk_d;                       // S X (FP64) during set-up, then T (and H T when 2 ss <= sd)
+  size_t off = 2 * blk_d;
+  if (2 * ss <= sd) w.ht = w.sx_t + blk_s; else { w.ht = off; off += blk_s; }
+  w.rx = off; off += blk_s;
+  w.ry = off; off += blk_s;
+  w.total = off;
+  return w;
+}
+
+pawfe_status ensure_scalars(pawfe_ctx* c, size_t doubles) {
+  if (doubles <= c->scal_doubles) return PAWFE_OK;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  cudaFree(c->d_scal);
+  c->h_pinned = nullptr; c->d_scal = nullptr; c->scal_doubles = 0;
+  size_t cap = std::max<size_t>(doubles, 64 * 512);
+  CUDA_TRY(c, cudaMallocHost((void**)&c->h_pinned, cap * pawfe_ctx::kScalSlots * sizeof(double)));
+  CUDA_TRY(c, cudaMalloc((void**)&c->d_scal, cap * pawfe_ctx::kScalSlots * sizeof(double)));
+  for (int i = 0; i < pawfe_ctx::kScalSlots; ++i)
+    if (!c->scal_ev[i]) CUDA_TRY(c, cudaEventCreateWithFlags(&c->scal_ev[i], cudaEventDisableTiming));
+  c->scal_doubles = cap;
+  return PAWFE_OK;
+}
+
+// TS: storage scalar (float / double / float2 / double2), TD: FP64 scalar of the same kind
+template <typename TS, typename TD>
+pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU, TS* X,
+                         const double* lambda, long ld, int B, void* workspace) {
+  typedef typename ScalarTraits<TS>::real RS;
+  const int cw = ScalarTraits<TS>::cplx ? 2 : 1;
+  const int W = B * cw;
+  const long total = c->M * (long)W;
+  WsLayout wl = ws_layout(c->M, B, sizeof(TS), sizeof(TD));
+  char* ws = (char*)workspace;
+  TD* Y64 = (TD*)(ws + wl.y64);
+  TD* SX64 = (TD*)(ws + wl.sx_t);
+  TS* T = (TS*)(ws + wl.sx_t);
+  TS* HT = (TS*)(ws + wl.ht);
+  TS* RX = (TS*)(ws + wl.rx);
+  TS* RY = (TS*)(ws + wl.ry);
+
+  // ---- step 1 and the Lambda recurrences, on the host in FP64 (L257, L264, L275) ----
+  const double e = 0.5 * (bU - bW), cc = 0.5 * (bU + bW);
+  double zeta = e / (b0 - cc);
+  const double gamma = 2.0 / zeta;
+  TRY(ensure_scalars(c, (size_t)(m + 1) * B));
+  const int slot = c->scal_next;
+  c->scal_next = (slot + 1) % pawfe_ctx::kScalSlots;
+  CUDA_TRY(c, cudaEventSynchronize(c->scal_ev[slot]));  // the slot's previous copy has been consumed
+  double* hs = c->h_pinned + (size_t)slot * c->scal_doubles;
+  double* ds = c->d_scal + (size_t)slot * c->scal_doubles;
+  std::vector<double> LX(B, 1.0), LY(B);
+  std::vector<double> as(m + 1, 0.0), acs(m + 1, 0.0), zzs(m + 1, 0.0);
+  const double z_over_e = zeta / e;
+  for (int v = 0; v < B; ++v) { hs[v] = lambda[v]; LY[v] = z_over_e * (lambda[v] - cc); }
+  for (int th = 2; th <= m; ++th) {
+    double zeta1 = 1.0 / (gamma - zeta);
+    double a = 2.0 * zeta1 / e;
+    as[th] = a; acs[th] = a * cc; zzs[th] = zeta * zeta1;
+    double* aL = hs + (size_t)(th - 1) * B;
+    for (int v = 0; v < B; ++v) {
+      aL[v] = a * LY[v];
+      double lx = a * LY[v] * lambda[v] - a * cc * LY[v] - zeta * zeta1 * LX[v];
+      LX[v] = LY[v]; LY[v] = lx;  // swap
+    }
+    zeta = zeta1;
+  }
+  for (int v = 0; v < B; ++v) hs[(size_t)m * B + v] = LY[v];
+  CUDA_TRY(c, cudaMemcpyAsync(ds, hs, (size_t)(m + 1) * B * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(c, cudaEventRecord(c->scal_ev[slot], c->stream));
+
+  // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
+  TRY((pawfe_apply_HS<TS, TD, TD>(c, 0, false, X, ld, Y64, B, B)));
+  TRY((pawfe_apply_HS<TS, TD, TD>(c, 1, false, X, ld, SX64, B, B)));
+  const int gs = 8 * c->sm_count;
+  // ---- step 3 ----
+  k_residual_init<RS><<<gs, 256, 0, c->stream>>>(c->M, W, cw, (double*)Y64, (const double*)SX64, ds, z_over_e,
+                                                 (RS*)RX, (RS*)RY);
+  KERNEL_CHECK(c, "k_residual_init");
+  // ---- step 4 ----
+  for (int th = 2; th <= m; ++th) {
+    TRY((pawfe_apply_Sinv_impl<TS, TS, TS>(c, RY, B, T, B, B)));
+    TRY(pawfe_apply_H_any(c, prec, T, B, HT, B, B));
+    k_recurrence<RS><<<gs, 256, 0, c->stream>>>(total, W, cw, (const RS*)HT, (const RS*)RY, (RS*)RX,
+                                                (const double*)Y64, ds + (size_t)(th - 1) * B, as[th], acs[th], zzs[th]);
+    KERNEL_CHECK(c, "k_recurrence");
+    std::swap(RX, RY);
+  }
+  // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y (L282) ----
+  TRY((pawfe_apply_Sinv_impl<TS, TS, TS>(c, RY, B, T, B, B)));
+  k_recover<RS><<<gs, 256, 0, c->stream>>>(c->md, W, cw, (const RS*)T, (RS*)X, ld * cw, ds + (size_t)m * B);
+  KERNEL_CHECK(c, "k_recover");
+  return PAWFE_OK;
+}
+
+pawfe_status check_filter(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU, const void* X,
+                          const double* lambda, long ld, int B) {
+  if (!c) return PAWFE_EINVAL;
+  if (!X || !lambda || B < 1 || B > 512 || ld < B || m < 1 || m > 512) { c->err = "bad filter arguments"; return PAWFE_EINVAL; }
+  if (!(bU > bW) || !(b0 < bW)) { c->err = "need b0 < bW < bU"; return PAWFE_EINVAL; }
+  if (prec != PAWFE_FP64 && prec != PAWFE_FP32 && prec != PAWFE_TF32) return PAWFE_EINVAL;
+  if (!c->have_mesh || !c->have_atoms || !c->have_pot) { c->err = "operators not set up"; return PAWFE_ESTATE; }
+  if (!c->have_h64) { c->err = "the filter's residual set-up needs the FP64 cell matrices (keep_fp64 = 1)"; return PAWFE_ESTATE; }
+  return PAWFE_OK;
+}
+
+}  // namespace
+
+extern "C" pawfe_status pawfe_filter_workspace(pawfe_ctx* c, pawfe_prec prec, int B, size_t* bytes) {
+  if (!c || !bytes || B < 1 || B > 512) return PAWFE_EINVAL;
+  if (!c->have_mesh) return PAWFE_ESTATE;
+  size_t cw = c->cplx ? 2 : 1;
+  size_t ss = (prec == PAWFE_FP64 ? 8 : 4) * cw, sd = 8 * cw;
+  *bytes = ws_layout(c->M, B, ss, sd).total;
+  return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                          void* X, const double* lambda, long ld, int B, void* workspace,
+                                          size_t workspace_bytes) {
+  TRY(check_filter(c, prec, m, b0, bW, bU, X, lambda, ld, B));
+  size_t need = 0;
+  TRY(pawfe_filter_workspace(c, prec, B, &need));
+  if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) { c->err = "workspace too small or misaligned"; return PAWFE_EINVAL; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  if (c->cplx) {
+    if (prec == PAWFE_FP64) return filter_impl<double2, double2>(c, prec, m, b0, bW, bU, (double2*)X, lambda, ld, B, workspace);
+    return filter_impl<float2, double2>(c, prec, m, b0, bW, bU, (float2*)X, lambda, ld, B, workspace);
+  }
+  if (prec == PAWFE_FP64) return filter_impl<double, double>(c, prec, m, b0, bW, bU, (double*)X, lambda, ld, B, workspace);
+  return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace);
+}
+
+extern "C" pawfe_status pawfe_cheb_filter_host(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW,
+                                               double bU, void* X_host, const double* lambda, long ld, int B) {
+  TRY(check_filter(c, prec, m, b0, bW, bU, X_host, lambda, ld, B));
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  size_t es = (prec == PAWFE_FP64 ? 8 : 4) * (c->cplx ? 2 : 1);
+  size_t blk = (size_t)c->M * ld * es, need = 0;
+  TRY(pawfe_filter_workspace(c, prec, B, &need));
+  if (blk > c->hostblk_bytes) {
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_hostblk); c->d_hostblk = nullptr; c->hostblk_bytes = 0;
+    char* p = nullptr; TRY(dev_alloc(c, &p, blk)); c->d_hostblk = p; c->hostblk_bytes = blk;
+  }
+  if (need > c->hostws_bytes) {
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_hostws); c->d_hostws = nullptr; c->hostws_bytes = 0;
+    char* p = nullptr; TRY(dev_alloc(c, &p, need)); c->d_hostws = p; c->hostws_bytes = need;
+  }
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_hostblk, X_host, blk, cudaMemcpyHostToDevice, c->stream));
+  TRY(pawfe_cheb_filter(c, prec, m, b0, bW, bU, c->d_hostblk, lambda, ld, B, c->d_hostws, c->hostws_bytes));
+  CUDA_TRY(c, cudaMemcpyAsync(X_host, c->d_hostblk, blk, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return PAWFE_OK;
+}

@@ -1,0 +1,14 @@
+// cell_tcgen05.h -- TF32 cell contraction Y_e = H^e T_e on tcgen05 tensor cores (PAPER.md:L347 step iii;
+// TF32: L11, L27).  Host-side entry points used by the API translation units.
+#pragma once
+#include "common.h"
+
+// Drop any cached tensor maps / plans (called when the cell matrices are rebuilt or freed).
+void tc_invalidate(pawfe_ctx* ctx);
+
+// True if the tensor-core kernel handles this context's (p, scalar type) and block width B.
+bool tc_supported(const pawfe_ctx* ctx, int B);
+
+// Y += alpha * sum_e P_e^T H^e (P_e X) for a real FP32 block, TF32 multiply, FP32 accumulate.
+// X, Y: device [dof][vec] float, leading dimensions ldx, ldy.  Y must already hold the values to add to.
+pawfe_status tc_cell_apply(pawfe_ctx* ctx, const float* X, long ldx, float* Y, long ldy, int B, float alpha);

@@ -1,0 +1,30 @@
+// host_util.h -- small host helpers shared by the API translation units.
+#pragma once
+#include "common.h"
+#include "cell_tcgen05.h"
+#include <new>
+
+template <typename T>
+static inline pawfe_status dev_alloc(pawfe_ctx* ctx, T** p, size_t count) {
+  *p = nullptr;
+  if (count == 0) return PAWFE_OK;
+  cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    ctx->err = std::string("cudaMalloc of ") + std::to_string(count * sizeof(T)) + " bytes: " + cudaGetErrorString(e);
+    return PAWFE_ENOMEM;
+  }
+  return PAWFE_OK;
+}
+#define TRY(x) do { pawfe_status s_ = (x); if (s_ != PAWFE_OK) return s_; } while (0)
+
+template <typename T>
+static inline pawfe_status upload(pawfe_ctx* ctx, T** d, const std::vector<T>& h) {
+  TRY(dev_alloc(ctx, d, h.size()));
+  CUDA_TRY(ctx, cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return PAWFE_OK;
+}
+
+void pawfe_free_mesh(pawfe_ctx* c);
+void pawfe_free_pot(pawfe_ctx* c);
+void pawfe_free_atoms(pawfe_ctx* c);

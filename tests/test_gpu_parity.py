@@ -1,0 +1,164 @@
+"""GPU parity: libpawfe.so (through the C ABI) against the FP64 CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's north_star: per product FP64 <= 1e-12, FP32 <= 1e-5,
+TF32 <= 5e-3 (relative Frobenius error on the seeded random block); FP64 filter call <= 1e-10.
+
+Cases: BASELINE.json configs[0] (full) and reduced-cell twins of configs 1-4 (same p, h, potential,
+projector set, boundary condition and k-point), sized so the oracle finishes in seconds while every
+kernel still sees several cells, vector tiles and a ragged tail.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from pawfe_inputs import get_config, make_system, random_block, twin  # noqa: E402
+
+TOL = {"fp64": 1e-12, "fp32": 1e-5, "tf32": 5e-3}
+
+
+def _cases():
+    return {
+        "cfg0": get_config(0),
+        "cfg1_twin": twin(get_config(1), nc=4, natoms=3, nvec=40, block=40, degree=6),
+        "cfg2_twin": twin(get_config(2), nc=4, natoms=3, nvec=24, block=24, degree=5),
+        "cfg3_twin": twin(get_config(3), nc=4, natoms=3, nvec=20, block=20, degree=5),
+        "cfg4_twin": twin(get_config(4), nc=4, natoms=3, nvec=24, block=24, degree=5),
+    }
+
+
+_CACHE = {}
+
+
+def _setup(name):
+    if name in _CACHE:
+        return _CACHE[name]
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from oracle.operators import PawOperators
+    from paper_2604_26037_b200 import context_from_system
+    cfg = _cases()[name]
+    sysd = make_system(cfg)
+    ops = PawOperators(sysd)
+    ctx = context_from_system(sysd, device=0, stream=torch.cuda.current_stream().cuda_stream)
+    _CACHE[name] = (cfg, sysd, ops, ctx)
+    return _CACHE[name]
+
+
+def _to_dev(x, prec, cplx):
+    """numpy (M, B) real/complex -> torch CUDA tensor in the library's element layout."""
+    real = np.float64 if prec == "fp64" else np.float32
+    if cplx:
+        a = np.stack([x.real, x.imag], axis=-1).astype(real)
+    else:
+        a = x.astype(real)
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _to_host(t, cplx):
+    a = t.cpu().numpy().astype(np.float64)
+    return a[..., 0] + 1j * a[..., 1] if cplx else a
+
+
+def _relerr(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+CASES = ["cfg0", "cfg1_twin", "cfg2_twin", "cfg3_twin", "cfg4_twin"]
+
+
+@pytest.mark.parametrize("name", CASES)
+def test_cell_matrices_and_couplings(name):
+    cfg, sysd, ops, ctx = _setup(name)
+    n = ops.mesh.n
+    for e in sorted({0, ops.mesh.ncell_total // 2, ops.mesh.ncell_total - 1}):
+        He = ops.H_cell(*ops.mesh.cell_coords(e))
+        got = ctx.get_cell_matrix(e, n)
+        assert _relerr(got, He) < 1e-13, (name, e)
+    got = ctx.get_sinv_coupling(cfg.natoms, cfg.nproj)
+    assert _relerr(got, ops.dSinv) < 1e-11
+    assert ctx.num_pairs() >= len(ops.pairs)
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32", "tf32"])
+@pytest.mark.parametrize("name", CASES)
+def test_apply_H_S_Sinv(name, prec):
+    from paper_2604_26037_b200 import PREC
+    cfg, sysd, ops, ctx = _setup(name)
+    B = cfg.block
+    X = random_block(cfg, B) * ops.mask[:, None]
+    Xd = _to_dev(X, prec, cfg.complex)
+    Yd = torch.empty_like(Xd)
+    for opname, fn, ref in (("H", ctx.apply_H, ops.apply_H), ("S", ctx.apply_S, ops.apply_S),
+                            ("Sinv", ctx.apply_Sinv, ops.apply_Sinv)):
+        Yd.fill_(float("nan"))
+        fn(PREC[prec], Xd, Yd, B, B)
+        torch.cuda.synchronize()
+        got = _to_host(Yd, cfg.complex)
+        want = ref(X) * ops.mask[:, None]
+        err = _relerr(got, want)
+        tol = TOL[prec] if not (opname != "H" and prec == "tf32") else TOL["fp32"]  # only the H contraction is TF32
+        assert err < tol, (name, prec, opname, err)
+
+
+@pytest.mark.parametrize("name", CASES)
+def test_apply_with_padded_ld_and_ignored_boundary(name):
+    """ld > B, and garbage in Dirichlet boundary rows of X must not change the result."""
+    from paper_2604_26037_b200 import FP64
+    cfg, sysd, ops, ctx = _setup(name)
+    B, ld = 5, 8
+    X = random_block(cfg, B, stream=3)
+    want = ops.apply_H(X * ops.mask[:, None]) * ops.mask[:, None]
+    Xp = np.zeros((X.shape[0], ld), dtype=X.dtype)
+    Xp[:, :B] = X  # boundary rows keep their random values
+    Xd = _to_dev(Xp, "fp64", cfg.complex)
+    Yd = torch.full_like(Xd, 7.0)
+    ctx.apply_H(FP64, Xd, Yd, ld, B)
+    torch.cuda.synchronize()
+    got = _to_host(Yd, cfg.complex)
+    assert _relerr(got[:, :B], want) < 1e-12
+    assert np.all(got[:, B:] == 7.0 * (1 + 1j if cfg.complex else 1))
+
+
+def _bounds(ops, lam):
+    from oracle.chfsi import lanczos_upper_bound
+    bU = lanczos_upper_bound(ops.apply_H, ops.apply_Sinv, ops.mesh.M, k=10, seed=1, dtype=ops.dtype, mask=ops.mask)
+    return lam[0] - 0.1, lam[-1] + 0.05, bU
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32", "tf32"])
+@pytest.mark.parametrize("name", CASES)
+def test_filter_call(name, prec):
+    """One Algorithm-2 call against the oracle's filter_residual on an S-orthonormal Ritz block."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import PREC
+    cfg, sysd, ops, ctx = _setup(name)
+    B, m = cfg.block, cfg.degree
+    X0 = random_block(cfg, B, stream=1) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+    Xd = _to_dev(X, prec, cfg.complex)
+    nbytes = ctx.filter_workspace(PREC[prec], B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(PREC[prec], m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    got = _to_host(Xd, cfg.complex)
+    err = _relerr(got, want)
+    tol = {"fp64": 1e-10, "fp32": 5e-4, "tf32": 5e-2}[prec]
+    assert err < tol, (name, prec, err)
+
+
+def test_col_norms():
+    from paper_2604_26037_b200 import FP32, FP64
+    cfg, sysd, ops, ctx = _setup("cfg3_twin")
+    B = 7
+    X = random_block(cfg, B, stream=5)
+    want = np.sqrt(np.sum(np.abs(X) ** 2, axis=0))
+    for prec, name in ((FP64, "fp64"), (FP32, "fp32")):
+        Xd = _to_dev(X, name, cfg.complex)
+        out = torch.zeros(B, dtype=torch.float64, device="cuda")
+        ctx.col_norms(prec, Xd, B, B, out)
+        torch.cuda.synchronize()
+        assert np.allclose(out.cpu().numpy(), want, rtol=1e-6 if name == "fp32" else 1e-13)
