@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- R-ChFSI filter throughput (dof x vector x Chebyshev-step per second) on B200.
+
+One "step" = one pass of the whole hot path (Algorithm 2: FP64 residual set-up, (m-1) x
+[S^-1approx, cell contraction + assembly, recurrence], recovery) over all N/B vector blocks of the
+workload = one "SCF-equivalent pass".  Workload at N=1: BASELINE.json configs[1] (16^3 cells, p=6,
+884,736 dofs, 400 vectors in blocks of 200, degree 20), synthetic seeded inputs.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 1] [--prec tf32]
+
+Multi-GPU: the path does not shard in this build ("replicas only"): under torchrun every rank
+filters its own replica of the workload on its own GPU; value = all ranks' units / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from pawfe_inputs import get_config, make_system, random_block, twin  # noqa: E402
+
+METRIC = "chfsi_filter_dof_vec_steps_per_s"
+UNIT = "dof*vec*steps/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sust=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sust=1400.0, src="fallback")
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline of the own arm, and the whole `--impl reference` arm)
+# ------------------------------------------------------------------------------------------------
+class OracleSample:
+    """A bounded sample of the workload for the CPU oracle: the reduced-cell twin of the config (same p, h,
+    potential, projector set, BC, k-point; 4^3 cells), B_o columns, m_o Chebyshev steps.  SpMM cost is
+    linear in dofs, columns and steps, so dof*vec*steps/s of the sample is the oracle's rate."""
+
+    def __init__(self, cfg_id: int, cols: int = 32, degree: int = 8):
+        from oracle import chfsi
+        from oracle.operators import PawOperators
+        self.chfsi = chfsi
+        base = get_config(cfg_id)
+        self.cfg = twin(base, nc=4, natoms=3, nvec=cols, block=cols, degree=degree)
+        self.ops = PawOperators(make_system(self.cfg))
+        ops = self.ops
+        X0 = random_block(self.cfg, cols, stream=7) * ops.mask[:, None]
+        X = chfsi.s_orthonormalise(ops.apply_S, X0)
+        self.X, self.lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+        self.bU = chfsi.lanczos_upper_bound(ops.apply_H, ops.apply_Sinv, ops.mesh.M, k=10, seed=1,
+                                            dtype=ops.dtype, mask=ops.mask)
+        self.units = float(ops.mesh.M) * cols * degree
+        self.desc = (f"oracle.chfsi.filter_residual (FP64, scipy CSR) on the {self.cfg.ncells[0]}^3-cell twin of "
+                     f"config {cfg_id} ({ops.mesh.M} dofs), {cols} vectors, degree {degree}; operators prebuilt")
+
+    def step(self):
+        o = self.ops
+        self.chfsi.filter_residual(o.apply_H, o.apply_S, o.apply_Sinv, self.X, self.lam, self.cfg.degree,
+                                   self.lam[0] - 0.1, self.lam[-1] + 0.05, self.bU)
+
+
+def _cores_used() -> int:
+    # scipy CSR products are single-threaded; the small dense numpy parts may use BLAS threads
+    return 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    smp = OracleSample(args.config)
+    for _ in range(max(1, min(args.warmup, 2))):
+        smp.step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        smp.step()
+    dt = time.perf_counter() - t0
+    val = smp.units * args.steps / dt
+    cfg = get_config(args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "sample": smp.desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": _cores_used(), "kind": "oracle", "sample": smp.desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in out.strip().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# own arm
+# ------------------------------------------------------------------------------------------------
+def run_own(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2604_26037_b200 import build
+    build.build()
+    from paper_2604_26037_b200 import PREC, FP64, context_from_system
+    from paper_2604_26037_b200.harness import Harness
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libpawfe has no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    prec = PREC[args.prec]
+    cfg = get_config(args.config)
+    sysd = make_system(cfg)
+    stream = torch.cuda.current_stream()
+    t_setup = time.perf_counter()
+    ctx = context_from_system(sysd, device=local, stream=stream.cuda_stream)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t_setup
+    M, N, B, m = ctx.num_dofs(), cfg.nvec, cfg.block, cfg.degree
+    cplx = cfg.complex
+    hz = Harness(ctx, M, cplx)
+    shape = (M, B, 2) if cplx else (M, B)
+    nblk = (N + B - 1) // B
+
+    # inputs: seeded U[-0.5, 0.5] blocks, S-orthonormalised per block, Ritz values
+    # from a per-block Rayleigh-Ritz, b_U from a 10-step Lanczos on H S^-1approx; all with the library's applies.
+    gen = torch.Generator(device=dev).manual_seed(cfg.seed + 1000 * rank)
+    blocks64, lams = [], []
+    for b in range(nblk):
+        X0 = torch.rand(shape, dtype=torch.float64, device=dev, generator=gen) - 0.5
+        X = hz.s_orthonormalise(X0)
+        X, lam = hz.rayleigh_ritz(X)
+        blocks64.append(X)
+        lams.append(lam)
+    bU = hz.upper_bound(k=10, seed=1)
+    b0 = min(l[0] for l in lams) - 0.1
+    bW = min(max(l[-1] for l in lams), 0.5 * (b0 + bU))
+    tdt = torch.float64 if prec == FP64 else torch.float32
+    ring_n = max(1, min(args.steps + args.warmup, args.ring))
+    ring = [[x.to(tdt).clone() for x in blocks64] for _ in range(ring_n)]
+    del blocks64
+    nbytes = ctx.filter_workspace(prec, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+
+    def one_step(i):
+        blks = ring[i % ring_n]
+        for b in range(nblk):
+            ctx.cheb_filter(prec, m, b0, bW, bU, blks[b], lams[b], B, B, ws, nbytes)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        one_step(i)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ctx.cell_timing(True)
+    l0 = ctx.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for i in range(args.steps):
+        one_step(args.warmup + i)
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    ncell_launch, cell_ms = ctx.cell_timing_read()
+    ctx.cell_timing(False)
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    finite = all(bool(torch.isfinite(x).all()) for blks in ring for x in blks)
+
+    # end to end through the C ABI with HOST buffers: H2D of each block, filter, D2H of Psi_f, inside the timed region
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    host_blocks = [x.cpu().pin_memory() for x in ring[0]]
+    one = lambda: [ctx.cheb_filter_host(prec, m, b0, bW, bU, hb.data_ptr(), lams[b], B, B) for b, hb in enumerate(host_blocks)]
+    one()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        one()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    blk_bytes = host_blocks[0].numel() * host_blocks[0].element_size()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    units = float(M) * N * m                      # per rank per step
+    value = world * units * args.steps / (ms * 1e-3)
+    peaks = _peaks()
+    n = (cfg.p + 1) ** 3
+    ncell = cfg.ncells[0] * cfg.ncells[1] * cfg.ncells[2]
+    flops_launch = 2.0 * n * n * B * ncell * (4 if cplx else 1)
+    cell_avg_ms = cell_ms / max(1, ncell_launch)
+    kname = ctx.cell_kernel_name(prec, B)
+    if "tcgen05" in kname:
+        peak = 0.5 * peaks["bf16_sust"]
+        peak_note = f"0.5 x {peaks['src']} sustained bf16 (TF32:bf16 nominal ratio)"
+        bound = "tensor"
+    else:
+        # SIMT FMA pipe: 148 SMs x 128 FP32 lanes x 2 flop at the clock seen under load
+        mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        peak = 148 * 128 * 2 * mhz * 1e6 / 1e12 * (0.5 if prec == FP64 else 1.0)
+        peak_note = "148 SM x 128 lanes x 2 flop x SM clock under load (FP64: half)"
+        bound = "alu"
+    achieved = flops_launch / (cell_avg_ms * 1e-3) / 1e12 if cell_avg_ms > 0 else 0.0
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {"fp64": "f64", "fp32": "f32", "tf32": "tf32"}[args.prec], "data": "synthetic",
+        "config": {"workload": cfg.name, "dofs": M, "vectors": N, "block": B, "degree": m, "precision": args.prec,
+                   "cells": ncell, "fe_order": cfg.p, "atoms": cfg.natoms, "projectors": cfg.nproj,
+                   "pairs": ctx.num_pairs(), "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "cache": f"inputs >> L2: ring of {ring_n} copies of the {N}-vector block set "
+                            f"({ring_n * nblk * blk_bytes / 2**30:.1f} GiB) + {nbytes / 2**30:.1f} GiB workspace per call",
+                   "bounds": [b0, bW, bU], "finite": finite, "setup_s": t_setup},
+        "clocks": clocks,
+        "e2e": {"value": world * units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nblk * blk_bytes,
+                "d2h_bytes_per_step": nblk * blk_bytes, "steps": e2e_steps},
+        "gpu_launches": launches,
+        "roofline": {"kernel": kname, "bound": bound, "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": None,
+                     "launches": ncell_launch, "avg_ms": cell_avg_ms, "share_of_step": cell_ms / ms,
+                     "peak_source": peak_note,
+                     "hbm_stream_gbs": (4.0 * n * n * ncell * (2 if cplx else 1)) / (cell_avg_ms * 1e-3) / 1e9 if cell_avg_ms > 0 else None},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        smp = OracleSample(args.config)
+        smp.step()
+        t0 = time.perf_counter()
+        reps = 0
+        while reps < 3 or (time.perf_counter() - t0 < 10.0 and reps < 50):
+            smp.step()
+            reps += 1
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": smp.units * reps / dt, "unit": UNIT, "cores": _cores_used(), "kind": "oracle",
+                                "sample": smp.desc + f"; {reps} calls in {dt:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="own", choices=["own", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--prec", default="tf32", choices=["fp64", "fp32", "tf32"])
+    ap.add_argument("--ring", type=int, default=8)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_own(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -163,6 +163,13 @@ pawfe_status pawfe_col_norms(pawfe_ctx* ctx, pawfe_prec prec, const void* X, lon
 /* Count of kernels this context has launched so far (bench.py's gpu_launches). */
 pawfe_status pawfe_launch_count(const pawfe_ctx* ctx, long* n);
 
+/* CUDA-event timing of the cell-contraction launches inside H S^-1approx (the FP32 / TF32 cell kernel of
+ * pawfe_apply_H and of step 4 of the filter): enable != 0 starts recording one event pair per launch on
+ * the context's stream and resets the counters; 0 stops.  pawfe_cell_timing_read synchronises the stream
+ * and returns the number of launches recorded and the sum of their durations in milliseconds. */
+pawfe_status pawfe_cell_timing(pawfe_ctx* ctx, int enable);
+pawfe_status pawfe_cell_timing_read(pawfe_ctx* ctx, long* launches, double* ms);
+
 /* Name of the cell-contraction kernel variant a given (prec, B) runs ("tcgen05_tf32", "simt_fp32",
  * "simt_fp64", ...).  Static string. */
 const char* pawfe_cell_kernel_name(const pawfe_ctx* ctx, pawfe_prec prec, int B);

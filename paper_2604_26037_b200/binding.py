@@ -26,7 +26,8 @@ SYMBOLS = [
     "pawfe_local_potential_gaussians", "pawfe_atoms_create", "pawfe_update_coupling", "pawfe_num_dofs",
     "pawfe_num_pairs", "pawfe_get_cell_matrix", "pawfe_get_sinv_coupling", "pawfe_apply_H", "pawfe_apply_S",
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host",
-    "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name",
+    "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
+    "pawfe_cell_timing_read",
 ]
 
 
@@ -70,6 +71,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
                                            C.c_long, C.c_int]
     lib.pawfe_col_norms.argtypes = [vp, C.c_int, vp, C.c_long, C.c_int, vp]
     lib.pawfe_launch_count.argtypes = [vp, C.POINTER(C.c_long)]
+    lib.pawfe_cell_timing.argtypes = [vp, C.c_int]
+    lib.pawfe_cell_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
     lib.pawfe_cell_kernel_name.argtypes = [vp, C.c_int, C.c_int]
     lib.pawfe_cell_kernel_name.restype = C.c_char_p
     for s in SYMBOLS:
@@ -169,6 +172,14 @@ class Context:
         v = C.c_long()
         self._check(self.lib.pawfe_launch_count(self._h, C.byref(v)), "pawfe_launch_count")
         return v.value
+
+    def cell_timing(self, enable: bool):
+        self._check(self.lib.pawfe_cell_timing(self._h, int(enable)), "pawfe_cell_timing")
+
+    def cell_timing_read(self):
+        n, ms = C.c_long(), C.c_double()
+        self._check(self.lib.pawfe_cell_timing_read(self._h, C.byref(n), C.byref(ms)), "pawfe_cell_timing_read")
+        return n.value, ms.value
 
     def cell_kernel_name(self, prec: int, B: int) -> str:
         return self.lib.pawfe_cell_kernel_name(self._h, int(prec), int(B)).decode()

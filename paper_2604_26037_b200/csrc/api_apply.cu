@@ -97,8 +97,13 @@ pawfe_status pawfe_apply_HS(pawfe_ctx* c, int op, bool tf32, const TX* X, long l
   TRY(zero_block(c, Y, ldy, B));
   const TC* A = op == 0 ? OpData<TC>::H(c) : OpData<TC>::Mref(c);
   long stride = op == 0 ? (long)c->n * OpData<TC>::lda(c) : 0;
-  if (tf32 && op == 0) TRY((launch_cell<TX, TY, TC, true>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0)));
-  else TRY((launch_cell<TX, TY, TC, false>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0)));
+  const bool timed = (op == 0) && sizeof(typename ScalarTraits<TC>::real) == 4;  // the loop's contraction
+  if (timed) prof_begin(c);
+  pawfe_status st;
+  if (tf32 && op == 0) st = launch_cell<TX, TY, TC, true>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0);
+  else st = launch_cell<TX, TY, TC, false>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0);
+  if (timed) prof_end(c);
+  TRY(st);
   const TC* Delta = op == 0 ? OpData<TC>::D(c) : OpData<TC>::dS(c);
   return pawfe_apply_nonlocal<TX, TY, TC>(c, Delta, 1.0, X, ldx, 0, Y, ldy, 0, B);
 }
@@ -171,7 +176,10 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
   if (c->cplx) return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
   if (tf32 && tc_supported(c, B)) {
     TRY(zero_block(c, (float*)Y, ldy, B));
-    TRY(tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f));
+    prof_begin(c);
+    pawfe_status st = tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f);
+    prof_end(c);
+    TRY(st);
     return pawfe_apply_nonlocal<float, float, float>(c, OpData<float>::D(c), 1.0, (const float*)X, ldx, 0, (float*)Y, ldy, 0, B);
   }
   return pawfe_apply_HS<float, float, float>(c, 0, tf32, (const float*)X, ldx, (float*)Y, ldy, B);
@@ -197,5 +205,26 @@ extern "C" pawfe_status pawfe_col_norms(pawfe_ctx* c, pawfe_prec prec, const voi
   KERNEL_CHECK(c, "k_col_sumsq");
   k_sqrt_inplace<<<ceil_div(B, 128), 128, 0, c->stream>>>(out, B);
   KERNEL_CHECK(c, "k_sqrt_inplace");
+  return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_cell_timing(pawfe_ctx* c, int enable) {
+  if (!c) return PAWFE_EINVAL;
+  c->prof_on = enable != 0;
+  c->prof_used = 0;
+  return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_cell_timing_read(pawfe_ctx* c, long* launches, double* ms) {
+  if (!c || !launches || !ms) return PAWFE_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < c->prof_used; i += 2) {
+    float t = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&t, c->prof_ev[i], c->prof_ev[i + 1]));
+    tot += t;
+  }
+  *launches = (long)(c->prof_used / 2);
+  *ms = tot;
   return PAWFE_OK;
 }

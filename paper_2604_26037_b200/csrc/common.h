@@ -178,6 +178,11 @@ struct pawfe_ctx {
   cudaEvent_t scal_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int scal_next = 0;
 
+  // optional CUDA-event timing of the cell-contraction launches of the filter loop (pawfe_cell_timing)
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_ev;  // pairs (start, stop)
+  size_t prof_used = 0;
+
   // host-buffer filter (pawfe_cheb_filter_host)
   void* d_hostblk = nullptr; size_t hostblk_bytes = 0;
   void* d_hostws = nullptr;  size_t hostws_bytes = 0;

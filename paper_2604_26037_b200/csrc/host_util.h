@@ -28,3 +28,19 @@ static inline pawfe_status upload(pawfe_ctx* ctx, T** d, const std::vector<T>& h
 void pawfe_free_mesh(pawfe_ctx* c);
 void pawfe_free_pot(pawfe_ctx* c);
 void pawfe_free_atoms(pawfe_ctx* c);
+
+// CUDA-event bracket around one cell-contraction launch (only when pawfe_cell_timing enabled it)
+static inline void prof_begin(pawfe_ctx* c) {
+  if (!c->prof_on) return;
+  if (c->prof_used + 2 > c->prof_ev.size()) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    c->prof_ev.push_back(a); c->prof_ev.push_back(b);
+  }
+  cudaEventRecord(c->prof_ev[c->prof_used], c->stream);
+}
+static inline void prof_end(pawfe_ctx* c) {
+  if (!c->prof_on) return;
+  cudaEventRecord(c->prof_ev[c->prof_used + 1], c->stream);
+  c->prof_used += 2;
+}

@@ -76,6 +76,7 @@ extern "C" pawfe_status pawfe_destroy(pawfe_ctx* c) {
   for (int i = 0; i < pawfe_ctx::kScalSlots; ++i) if (c->scal_ev[i]) cudaEventDestroy(c->scal_ev[i]);
   cudaFree(c->d_hostblk); cudaFree(c->d_hostws);
   if (c->h_stage) cudaFreeHost(c->h_stage);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
   return PAWFE_OK;
 }
