@@ -62,7 +62,11 @@ pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, c
   constexpr int BV = (sizeof(TC) == 16) ? 16 : 32;
   size_t smem = (size_t)c->n * 16 + (size_t)c->n * BV * sizeof(TC);
   auto kern = k_cell_simt<TX, TY, TC, BV, TF32>;
-  CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  static size_t smem_attr = 0;  // per instantiation; the attribute is per function, so only ever raise it
+  if (smem > smem_attr) {
+    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    smem_attr = smem;
+  }
   kern<<<dim3(c->ncell, ceil_div(B, BV)), 256, smem, c->stream>>>(c->md, A, cell_stride, lda, X, ldx, Y, ldy, B,
                                                                   in_scale, alpha);
   KERNEL_CHECK(c, "k_cell_simt");
@@ -174,7 +178,7 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
   }
   bool tf32 = prec == PAWFE_TF32;
   if (c->cplx) return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
-  if (tf32 && tc_supported(c, B)) {
+  if (tf32 && tc_usable(c, X, ldx, Y, ldy, B)) {
     TRY(zero_block(c, (float*)Y, ldy, B));
     prof_begin(c);
     pawfe_status st = tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f);

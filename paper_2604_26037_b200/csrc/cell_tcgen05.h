@@ -9,6 +9,10 @@ void tc_invalidate(pawfe_ctx* ctx);
 // True if the tensor-core kernel handles this context's (p, scalar type) and block width B.
 bool tc_supported(const pawfe_ctx* ctx, int B);
 
+// True if, in addition, these blocks meet the kernel's alignment rules (16-byte aligned pointers, leading
+// dimensions and B multiples of 4) and the tensor map could be built.
+bool tc_usable(pawfe_ctx* ctx, const void* X, long ldx, const void* Y, long ldy, int B);
+
 // Y += alpha * sum_e P_e^T H^e (P_e X) for a real FP32 block, TF32 multiply, FP32 accumulate.
 // X, Y: device [dof][vec] float, leading dimensions ldx, ldy.  Y must already hold the values to add to.
 pawfe_status tc_cell_apply(pawfe_ctx* ctx, const float* X, long ldx, float* Y, long ldy, int B, float alpha);

@@ -178,6 +178,8 @@ struct pawfe_ctx {
   cudaEvent_t scal_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int scal_next = 0;
 
+  void* tc_plan = nullptr;  // cell_tcgen05.cu: cached tensor map and tile shape
+
   // optional CUDA-event timing of the cell-contraction launches of the filter loop (pawfe_cell_timing)
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;  // pairs (start, stop)
