@@ -7,6 +7,7 @@
 #include "kernels_stream.cuh"
 #include "api_internal.h"
 #include "apply_impl.h"
+#include "fused.h"
 #include <algorithm>
 
 namespace {
@@ -178,6 +179,8 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
   }
   bool tf32 = prec == PAWFE_TF32;
   if (c->cplx) return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
+  if (tf32 && tc_usable(c, X, ldx, Y, ldy, B) && fused_supported(c, prec, B))
+    return fused_apply_H(c, (const float*)X, ldx, (float*)Y, ldy, B);
   if (tf32 && tc_usable(c, X, ldx, Y, ldy, B)) {
     TRY(zero_block(c, (float*)Y, ldy, B));
     prof_begin(c);

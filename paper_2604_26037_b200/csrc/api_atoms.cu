@@ -83,6 +83,7 @@ pawfe_status pawfe_upload_couplings(pawfe_ctx* c, const double* D, const double*
       if (cw == 2) vI[(a * per + i) * cw + 1] = X[2 * i + 1];
     }
   }
+  c->h_dSinv = vI;
   if (D) TRY((upload_coupling_arrays<double, float>(c, vD, &c->d_D64, &c->d_D32)));
   TRY((upload_coupling_arrays<double, float>(c, vS, &c->d_dS64, &c->d_dS32)));
   TRY((upload_coupling_arrays<double, float>(c, vI, &c->d_dSinv64, &c->d_dSinv32)));

@@ -6,6 +6,7 @@
 #include "kernels_stream.cuh"
 #include "api_internal.h"
 #include "apply_impl.h"
+#include "fused.h"
 #include <algorithm>
 #include <cstring>
 
@@ -20,7 +21,8 @@ struct WsLayout {
 // storage bytes per scalar: ss (4/8 real, 8/16 complex); FP64 scalar bytes: sd
 WsLayout ws_layout(long M, int B, size_t ss, size_t sd) {
   WsLayout w;
-  size_t blk_s = align256((size_t)M * B * ss), blk_d = align256((size_t)M * B * sd);
+  const size_t ldw = ((size_t)B + 3) / 4 * 4;  // the fused path pads rows to a multiple of 4 elements
+  size_t blk_s = align256((size_t)M * ldw * ss), blk_d = align256((size_t)M * ldw * sd);
   if (2 * ss <= sd) blk_d = std::max(blk_d, 2 * blk_s);
   w.y64 = 0;
   w.sx_t = blk_d;                       // S X (FP64) during set-up, then T (and H T when 2 ss <= sd)
@@ -47,6 +49,49 @@ pawfe_status ensure_scalars(pawfe_ctx* c, size_t doubles) {
   return PAWFE_OK;
 }
 
+// Step 1 and the Lambda recurrences of Alg. 2 on the host in FP64 (L257, L264, L275).  Fills a pinned staging slot,
+// starts its copy to the device and returns the per-step coefficients:
+//   device scalars ds: [0, B) Lambda;  [(th-1) B, th B) a_th Lambda_Y (th = 2..m);  [m B, (m+1) B) final Lambda_Y
+struct FilterScalars {
+  const double* ds = nullptr;
+  std::vector<double> as, acs, zzs;
+  double z_over_e = 0.0;
+};
+
+pawfe_status filter_scalars(pawfe_ctx* c, int m, double b0, double bW, double bU, const double* lambda, int B,
+                            FilterScalars* out) {
+  const double e = 0.5 * (bU - bW), cc = 0.5 * (bU + bW);
+  double zeta = e / (b0 - cc);
+  const double gamma = 2.0 / zeta;
+  TRY(ensure_scalars(c, (size_t)(m + 1) * B));
+  const int slot = c->scal_next;
+  c->scal_next = (slot + 1) % pawfe_ctx::kScalSlots;
+  CUDA_TRY(c, cudaEventSynchronize(c->scal_ev[slot]));  // the slot's previous copy has been consumed
+  double* hs = c->h_pinned + (size_t)slot * c->scal_doubles;
+  double* ds = c->d_scal + (size_t)slot * c->scal_doubles;
+  std::vector<double> LX(B, 1.0), LY(B);
+  out->as.assign(m + 1, 0.0); out->acs.assign(m + 1, 0.0); out->zzs.assign(m + 1, 0.0);
+  const double z_over_e = zeta / e;
+  for (int v = 0; v < B; ++v) { hs[v] = lambda[v]; LY[v] = z_over_e * (lambda[v] - cc); }
+  for (int th = 2; th <= m; ++th) {
+    double zeta1 = 1.0 / (gamma - zeta);
+    double a = 2.0 * zeta1 / e;
+    out->as[th] = a; out->acs[th] = a * cc; out->zzs[th] = zeta * zeta1;
+    double* aL = hs + (size_t)(th - 1) * B;
+    for (int v = 0; v < B; ++v) {
+      aL[v] = a * LY[v];
+      double lx = a * LY[v] * lambda[v] - a * cc * LY[v] - zeta * zeta1 * LX[v];
+      LX[v] = LY[v]; LY[v] = lx;  // swap
+    }
+    zeta = zeta1;
+  }
+  for (int v = 0; v < B; ++v) hs[(size_t)m * B + v] = LY[v];
+  CUDA_TRY(c, cudaMemcpyAsync(ds, hs, (size_t)(m + 1) * B * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(c, cudaEventRecord(c->scal_ev[slot], c->stream));
+  out->ds = ds; out->z_over_e = z_over_e;
+  return PAWFE_OK;
+}
+
 // TS: storage scalar (float / double / float2 / double2), TD: FP64 scalar of the same kind
 template <typename TS, typename TD>
 pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU, TS* X,
@@ -64,35 +109,11 @@ pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double
   TS* RX = (TS*)(ws + wl.rx);
   TS* RY = (TS*)(ws + wl.ry);
 
-  // ---- step 1 and the Lambda recurrences, on the host in FP64 (L257, L264, L275) ----
-  const double e = 0.5 * (bU - bW), cc = 0.5 * (bU + bW);
-  double zeta = e / (b0 - cc);
-  const double gamma = 2.0 / zeta;
-  TRY(ensure_scalars(c, (size_t)(m + 1) * B));
-  const int slot = c->scal_next;
-  c->scal_next = (slot + 1) % pawfe_ctx::kScalSlots;
-  CUDA_TRY(c, cudaEventSynchronize(c->scal_ev[slot]));  // the slot's previous copy has been consumed
-  double* hs = c->h_pinned + (size_t)slot * c->scal_doubles;
-  double* ds = c->d_scal + (size_t)slot * c->scal_doubles;
-  std::vector<double> LX(B, 1.0), LY(B);
-  std::vector<double> as(m + 1, 0.0), acs(m + 1, 0.0), zzs(m + 1, 0.0);
-  const double z_over_e = zeta / e;
-  for (int v = 0; v < B; ++v) { hs[v] = lambda[v]; LY[v] = z_over_e * (lambda[v] - cc); }
-  for (int th = 2; th <= m; ++th) {
-    double zeta1 = 1.0 / (gamma - zeta);
-    double a = 2.0 * zeta1 / e;
-    as[th] = a; acs[th] = a * cc; zzs[th] = zeta * zeta1;
-    double* aL = hs + (size_t)(th - 1) * B;
-    for (int v = 0; v < B; ++v) {
-      aL[v] = a * LY[v];
-      double lx = a * LY[v] * lambda[v] - a * cc * LY[v] - zeta * zeta1 * LX[v];
-      LX[v] = LY[v]; LY[v] = lx;  // swap
-    }
-    zeta = zeta1;
-  }
-  for (int v = 0; v < B; ++v) hs[(size_t)m * B + v] = LY[v];
-  CUDA_TRY(c, cudaMemcpyAsync(ds, hs, (size_t)(m + 1) * B * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-  CUDA_TRY(c, cudaEventRecord(c->scal_ev[slot], c->stream));
+  FilterScalars fs;
+  TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
+  const double* ds = fs.ds;
+  const std::vector<double>&as = fs.as, &acs = fs.acs, &zzs = fs.zzs;
+  const double z_over_e = fs.z_over_e;
 
   // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
   TRY((pawfe_apply_HS<TS, TD, TD>(c, 0, false, X, ld, Y64, B, B)));
@@ -153,6 +174,11 @@ extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, 
     return filter_impl<float2, double2>(c, prec, m, b0, bW, bU, (float2*)X, lambda, ld, B, workspace);
   }
   if (prec == PAWFE_FP64) return filter_impl<double, double>(c, prec, m, b0, bW, bU, (double*)X, lambda, ld, B, workspace);
+  if (fused_supported(c, prec, B)) {
+    FilterScalars fs;
+    TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
+    return fused_filter_real(c, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, (float*)X, ld, B, workspace);
+  }
   return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace);
 }
 

@@ -1,0 +1,596 @@
+// api_fused.cu -- fused Chebyshev step of Algorithm 2 for real FP32-storage blocks (see fused.h, DESIGN.md
+// "Fused step"): plan construction (K-extension blocks, neighbour couplings), the atom-local projection and
+// coupling kernels (Fig. 2 step ii; Eq. 28-29), the bracket prepass (L272, L374), recovery (L282).
+#include "fused.h"
+#include "cell_tcgen05.h"
+#include "host_util.h"
+#include "api_internal.h"
+#include "apply_impl.h"
+#include <algorithm>
+#include <cmath>
+#include <set>
+
+struct FusedPlan {
+  bool ok = false;
+  long nchunks = 0;
+  int* d_ext_start = nullptr;   // [ncell + 1]
+  int* d_ext_atom = nullptr;    // [nchunks]
+  float* d_Bext = nullptr;      // [nchunks][n][32]
+  int* d_nb_start = nullptr;    // [natoms + 1]
+  int* d_nb_atom = nullptr;     // [nnb]
+  float* d_GD = nullptr;        // [nnb][npj][npj]:  G^{ab} Delta^b_Sinv
+  int ext_ksteps = 4;
+  // scratch for block width <= Bcap
+  int Bcap = 0; long ldw = 0;
+  float* d_P1 = nullptr;        // [natoms][npj][ldw]
+  float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
+};
+
+namespace {
+
+inline long roundup4(long x) { return (x + 3) / 4 * 4; }
+
+// ---- pair lookup: index of (atom, cell) in the pair list (pairs sorted by atom, then cell), or -1 ----
+__device__ inline int find_pair(const int* __restrict__ aps, const int* __restrict__ pair_cell, int atom, int cell) {
+  int lo = aps[atom], hi = aps[atom + 1] - 1;
+  while (lo <= hi) {
+    int mid = (lo + hi) >> 1, pc = pair_cell[mid];
+    if (pc == cell) return mid;
+    if (pc < cell) lo = mid + 1; else hi = mid - 1;
+  }
+  return -1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Set-up: one CTA per K-extension chunk x = (cell e, atom b).
+//   Zs[I][be] = M_D^-1[J] * (assembled C^b)[J][be] at the nodes J of cell e  (sum over the <= 8 cells sharing J)
+//   Bext[x][I][be]       = - sum_J H^e[I][J] Zs[J][be]                         (be < npj)
+//   Bext[x][I][npj + be] = C^{e,b}[I][be] if (e, b) is a pair, else 0
+//   G[slot(a, b)][al][be] += sum_I C^{e,a}[I][al] Zs[I][be]   for every pair (e, a)     (G^{ab} = C^a^T M_D^-1 C^b)
+// Real contexts only.  block = 256; dynamic smem: n * npj doubles.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict__ ext_atom,
+            const int* __restrict__ aps, const int* __restrict__ pair_cell, const double* __restrict__ Cd64,
+            int npj, const double* __restrict__ H64, const int* __restrict__ cell_pair_start,
+            const int* __restrict__ cell_pair_idx, const int* __restrict__ pair_atom,
+            const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
+            float* __restrict__ Bext, double* __restrict__ G) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* Zs = reinterpret_cast<double*>(smem_raw);  // [n][npj]
+  const int n = md.n, n1 = md.n1, p = md.p;
+  const int x = blockIdx.x;
+  const int e = ext_cell[x], b = ext_atom[x];
+  int cx, cy, cz;
+  mesh_cell_coords(md, e, &cx, &cy, &cz);
+  const int cc[3] = {cx, cy, cz};
+  // ---- phase 1: assembled, M_D^-1-scaled projector values of atom b at this cell's nodes ----
+  for (int I = threadIdx.x; I < n; I += blockDim.x) {
+    const int loc[3] = {I / (n1 * n1), (I / n1) % n1, I % n1};
+    int ix, iy, iz;
+    mesh_node(md, cx, cy, cz, loc[0], loc[1], loc[2], &ix, &iy, &iz);
+    const double mi = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
+    // incidences of this node: per direction the own cell, plus the neighbour across a face the node lies on
+    int ncand[3], ccell[3][2], cloc[3][2];
+    for (int d = 0; d < 3; ++d) {
+      ncand[d] = 1; ccell[d][0] = cc[d]; cloc[d][0] = loc[d];
+      if (loc[d] == 0 || loc[d] == p) {
+        int nbc = loc[d] == 0 ? cc[d] - 1 : cc[d] + 1;
+        const int nbl = loc[d] == 0 ? p : 0;
+        if (md.periodic) nbc = (nbc + md.nc[d]) % md.nc[d];
+        if (nbc >= 0 && nbc < md.nc[d]) { ccell[d][1] = nbc; cloc[d][1] = nbl; ncand[d] = 2; }
+      }
+    }
+    for (int be = 0; be < npj; ++be) Zs[I * npj + be] = 0.0;
+    if (mi != 0.0) {
+      for (int qx = 0; qx < ncand[0]; ++qx)
+        for (int qy = 0; qy < ncand[1]; ++qy)
+          for (int qz = 0; qz < ncand[2]; ++qz) {
+            const int e2 = (ccell[0][qx] * md.nc[1] + ccell[1][qy]) * md.nc[2] + ccell[2][qz];
+            const int pr = find_pair(aps, pair_cell, b, e2);
+            if (pr < 0) continue;
+            const int I2 = (cloc[0][qx] * n1 + cloc[1][qy]) * n1 + cloc[2][qz];
+            for (int be = 0; be < npj; ++be) Zs[I * npj + be] += Cd64[((long)pr * npj + be) * n + I2];
+          }
+      for (int be = 0; be < npj; ++be) Zs[I * npj + be] *= mi;
+    }
+  }
+  __syncthreads();
+  // ---- phase 2: K-extension block ----
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int prb = find_pair(aps, pair_cell, b, e);
+  const double* He = H64 + (long)e * n * n;
+  float* Bx = Bext + (long)x * n * 32;
+  for (int I = w; I < n; I += nw) {
+    double acc[PAWFE_MAX_NPJ];
+#pragma unroll
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) acc[be] = 0.0;
+    for (int J = lane; J < n; J += 32) {
+      const double h = He[(long)I * n + J];
+#pragma unroll
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
+        if (be < npj) acc[be] = fma(h, Zs[J * npj + be], acc[be]);
+    }
+#pragma unroll
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
+      if (be < npj) {
+        double s = acc[be];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) Bx[I * 32 + be] = (float)(-s);
+      }
+    for (int k = npj + lane; k < 32; k += 32) {
+      float v = 0.f;
+      if (k < 2 * npj && prb >= 0) v = (float)Cd64[((long)prb * npj + (k - npj)) * n + I];
+      Bx[I * 32 + k] = v;
+    }
+  }
+  // ---- phase 3: G^{ab} contributions of this cell ----
+  for (int q = cell_pair_start[e]; q < cell_pair_start[e + 1]; ++q) {
+    const int pr = cell_pair_idx[q], a = pair_atom[pr];
+    int slot = -1;
+    for (int s = nb_start[a]; s < nb_start[a + 1]; ++s) if (nb_atom[s] == b) { slot = s; break; }
+    if (slot < 0) continue;
+    for (int ab = w; ab < npj * npj; ab += nw) {
+      const int al = ab / npj, be = ab % npj;
+      double s = 0.0;
+      for (int I = lane; I < n; I += 32) s = fma(Cd64[((long)pr * npj + al) * n + I], Zs[I * npj + be], s);
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (lane == 0) atomicAdd(&G[((long)slot * npj + al) * npj + be], s);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// (ii) partial non-local projection, pair-parallel:  P[a][al][v] += sum_I C^{e,a}[I][al] X[J(e,I)][v]
+//   grid = (npairs, ceil(B/128)), block = 256 (8 warps over rows, lane = 4 consecutive vectors).
+//   dynamic smem: n longs + npj*n floats + 16*128 floats.  P must be zero on entry.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
+        const float* __restrict__ Cd, int npj, const float* __restrict__ X, long ldx, int B,
+        float* __restrict__ P, long ldp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = md.n, n1 = md.n1;
+  long* nodeJ = reinterpret_cast<long*>(smem_raw);
+  float* Cs = reinterpret_cast<float*>(nodeJ + n);     // [npj][n]
+  float* red = Cs + (size_t)npj * n;                   // [16][128]
+  const int pr = blockIdx.x, a = pair_atom[pr];
+  int cx, cy, cz;
+  mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
+  for (int I = threadIdx.x; I < n; I += blockDim.x) {
+    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+    long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+    if (md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0) J = -1;
+    nodeJ[I] = J;
+  }
+  for (int i = threadIdx.x; i < npj * n; i += blockDim.x) Cs[i] = Cd[(long)pr * npj * n + i];
+  for (int i = threadIdx.x; i < 16 * 128; i += blockDim.x) red[i] = 0.f;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int v = blockIdx.y * 128 + lane * 4;
+  float4 acc[PAWFE_MAX_NPJ];
+#pragma unroll
+  for (int al = 0; al < PAWFE_MAX_NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (v < B) {
+#pragma unroll 4
+    for (int I = w; I < n; I += 8) {
+      const long J = nodeJ[I];
+      if (J < 0) continue;
+      const float4 x = __ldg(reinterpret_cast<const float4*>(X + J * ldx + v));
+#pragma unroll
+      for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
+        if (al < npj) {
+          const float cv = Cs[al * n + I];
+          acc[al].x = fmaf(cv, x.x, acc[al].x); acc[al].y = fmaf(cv, x.y, acc[al].y);
+          acc[al].z = fmaf(cv, x.z, acc[al].z); acc[al].w = fmaf(cv, x.w, acc[al].w);
+        }
+    }
+#pragma unroll
+    for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
+      if (al < npj) {
+        float* r = red + al * 128 + lane * 4;
+        atomicAdd(r + 0, acc[al].x); atomicAdd(r + 1, acc[al].y); atomicAdd(r + 2, acc[al].z); atomicAdd(r + 3, acc[al].w);
+      }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < npj * 128; i += blockDim.x) {
+    const int al = i >> 7, vv = blockIdx.y * 128 + (i & 127);
+    if (vv < B) atomicAdd(P + ((long)a * npj + al) * ldp + vv, red[i]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Couplings per atom and vector (Eq. 28-29, Eq. 16):
+//   W^a = Delta^a_Sinv P1^a;  P2^a = P1^a - sum_{b in nb(a)} (G^{ab} Delta^b_Sinv) P1^b;  W2^a = D^a P2^a.
+//   mode 0: both (filter step);  mode 1: W only (recovery, S^-1approx alone);  mode 2: plain H (W = 0, W2 = D P1).
+//   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2.  grid = (natoms, ceil(B/128)), block = 128.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_couple(int npj, int mode, const float* __restrict__ P1, long ldp, int B, const float* __restrict__ dSinv,
+         const float* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
+         const float* __restrict__ GD, float* __restrict__ Wcat, long ldw) {
+  const int a = blockIdx.x;
+  const int v = blockIdx.y * blockDim.x + threadIdx.x;
+  if (v >= B) return;
+  float p1[PAWFE_MAX_NPJ], p2[PAWFE_MAX_NPJ];
+#pragma unroll
+  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) { p1[be] = be < npj ? P1[((long)a * npj + be) * ldp + v] : 0.f; p2[be] = p1[be]; }
+  float* Wa = Wcat + (long)a * 32 * ldw;
+  if (mode != 2) {
+    const float* S = dSinv + (long)a * npj * npj;
+    for (int al = 0; al < npj; ++al) {
+      float s = 0.f;
+#pragma unroll
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s = fmaf(S[al * npj + be], p1[be], s);
+      Wa[(long)al * ldw + v] = s;
+    }
+  } else {
+    for (int al = 0; al < npj; ++al) Wa[(long)al * ldw + v] = 0.f;
+  }
+  if (mode == 1) return;
+  if (mode == 0) {
+    for (int s = nb_start[a]; s < nb_start[a + 1]; ++s) {
+      const int b = nb_atom[s];
+      const float* g = GD + (long)s * npj * npj;
+      float pb[PAWFE_MAX_NPJ];
+#pragma unroll
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) pb[be] = be < npj ? P1[((long)b * npj + be) * ldp + v] : 0.f;
+#pragma unroll
+      for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
+        if (al < npj) {
+          float t = 0.f;
+#pragma unroll
+          for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) t = fmaf(g[al * npj + be], pb[be], t);
+          p2[al] -= t;
+        }
+    }
+  }
+  const float* Da = D + (long)a * npj * npj;
+  for (int al = 0; al < npj; ++al) {
+    float s = 0.f;
+#pragma unroll
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s = fmaf(Da[al * npj + be], p2[be], s);
+    Wa[(long)(npj + al) * ldw + v] = s;
+  }
+}
+
+// X[J][v] += scale * M_D^-1[J] * sum_al C^{e,a}[I][al] W^a[al][v] over the pairs (recovery: scale = -1).
+//   grid = (npairs, ceil(B/128)), block = 256.  dynamic smem: n longs + n floats + npj*n floats.
+__global__ void __launch_bounds__(256)
+k_scatter2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
+           const float* __restrict__ Cd, int npj, const float* __restrict__ Wcat, long ldw, int B, float scale,
+           float* __restrict__ X, long ldx) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = md.n, n1 = md.n1;
+  long* nodeJ = reinterpret_cast<long*>(smem_raw);
+  float* nodeS = reinterpret_cast<float*>(nodeJ + n);
+  float* Cs = nodeS + n;
+  const int pr = blockIdx.x, a = pair_atom[pr];
+  int cx, cy, cz;
+  mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
+  for (int I = threadIdx.x; I < n; I += blockDim.x) {
+    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+    nodeJ[I] = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+    nodeS[I] = scale * (float)(md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz]);
+  }
+  for (int i = threadIdx.x; i < npj * n; i += blockDim.x) Cs[i] = Cd[(long)pr * npj * n + i];
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int v = blockIdx.y * 128 + lane * 4;
+  if (v >= B) return;
+  float4 wv[PAWFE_MAX_NPJ];
+#pragma unroll
+  for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
+    wv[al] = al < npj ? *reinterpret_cast<const float4*>(Wcat + ((long)a * 32 + al) * ldw + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int I = w; I < n; I += 8) {
+    const float s = nodeS[I];
+    if (s == 0.f) continue;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
+      if (al < npj) {
+        const float cv = Cs[al * n + I];
+        acc.x = fmaf(cv, wv[al].x, acc.x); acc.y = fmaf(cv, wv[al].y, acc.y);
+        acc.z = fmaf(cv, wv[al].z, acc.z); acc.w = fmaf(cv, wv[al].w, acc.w);
+      }
+    float* dst = X + nodeJ[I] * ldx + v;
+    atomicAdd(dst + 0, s * acc.x);
+    if (v + 1 < B) atomicAdd(dst + 1, s * acc.y);
+    if (v + 2 < B) atomicAdd(dst + 2, s * acc.z);
+    if (v + 3 < B) atomicAdd(dst + 3, s * acc.w);
+  }
+}
+
+__device__ inline double mdinv_row(const MeshDev& md, long J) {
+  int iz = (int)(J % md.N[2]);
+  long t = J / md.N[2];
+  int iy = (int)(t % md.N[1]);
+  int ix = (int)(t / md.N[1]);
+  return md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
+}
+
+// Alg. 2 steps 2-3 (L260-L264) in the scaled variables:  Yt = M_D^-1 (HX - SX Lambda) (FP64, in place in HX);
+// Rt_Y = (zeta/e) Yt;  Rt_X = 0.  All arrays have leading dimension ldw; pad columns are written as 0.
+__global__ void k_residual_init2(MeshDev md, long ldw, int B, double* __restrict__ HX, const double* __restrict__ SX,
+                                 const double* __restrict__ lam, double z_over_e, float* __restrict__ RX,
+                                 float* __restrict__ RY) {
+  const long total = md.M * ldw;
+  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+    const long J = idx / ldw;
+    const int v = (int)(idx - J * ldw);
+    double y = 0.0;
+    if (v < B) y = mdinv_row(md, J) * (HX[idx] - SX[idx] * lam[v]);
+    HX[idx] = y;
+    RY[idx] = (float)(z_over_e * y);
+    RX[idx] = 0.f;
+  }
+}
+
+// Bracket of Alg. 2 step 4 (L272) without the H term:  Rt_X <- (-a c) Rt_Y - (zeta zeta1) Rt_X  [FP32]
+//                                                           + Yt (a Lambda_Y)                  [FP64 add, L374]
+// 4 consecutive vectors per thread; ldw % 4 == 0.
+__global__ void __launch_bounds__(256)
+k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, float4* __restrict__ RX,
+          const double2* __restrict__ Yt, const double* __restrict__ aLamY, int B, float ac, float zz1) {
+  for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < nquads; q += (long)gridDim.x * blockDim.x) {
+    const int v = (int)(q % ldq) * 4;
+    const float4 ry = RY[q];
+    const float4 rx = RX[q];
+    const double2 y0 = Yt[2 * q], y1 = Yt[2 * q + 1];
+    double l0 = 0, l1 = 0, l2 = 0, l3 = 0;
+    if (v < B) l0 = aLamY[v];
+    if (v + 1 < B) l1 = aLamY[v + 1];
+    if (v + 2 < B) l2 = aLamY[v + 2];
+    if (v + 3 < B) l3 = aLamY[v + 3];
+    float4 o;
+    o.x = (float)((double)(-ac * ry.x - zz1 * rx.x) + y0.x * l0);
+    o.y = (float)((double)(-ac * ry.y - zz1 * rx.y) + y0.y * l1);
+    o.z = (float)((double)(-ac * ry.z - zz1 * rx.z) + y1.x * l2);
+    o.w = (float)((double)(-ac * ry.w - zz1 * rx.w) + y1.y * l3);
+    RX[q] = o;
+  }
+}
+
+// Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
+// by k_scatter2.  keep = 0 on Dirichlet boundary rows.
+__global__ void k_recover2(MeshDev md, long ldw, int B, const float* __restrict__ RY, float* __restrict__ X, long ldx,
+                           const double* __restrict__ lamY) {
+  const long total = md.M * (long)B;
+  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+    const long J = idx / B;
+    const int v = (int)(idx - J * B);
+    const double keep = mdinv_row(md, J) != 0.0 ? 1.0 : 0.0;
+    const double x = (double)X[J * ldx + v];
+    X[J * ldx + v] = (float)(keep * ((double)RY[J * ldw + v] + x * lamY[v]));
+  }
+}
+
+void free_plan(FusedPlan* p) {
+  if (!p) return;
+  cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
+  cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD);
+  cudaFree(p->d_P1); cudaFree(p->d_Wcat);
+  delete p;
+}
+
+pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
+  const int ncell = c->ncell, natoms = c->natoms, npj = c->npj, n = c->n;
+  const bool per = c->bc == PAWFE_PERIODIC;
+  // host copies of the pair list
+  std::vector<int> pc(c->npairs), pa(c->npairs);
+  if (c->npairs) {
+    CUDA_TRY(c, cudaMemcpy(pc.data(), c->d_pair_cell, c->npairs * sizeof(int), cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(pa.data(), c->d_pair_atom, c->npairs * sizeof(int), cudaMemcpyDeviceToHost));
+  }
+  // cell -> pairs
+  std::vector<int> cps(ncell + 1, 0), cpi(c->npairs);
+  for (long q = 0; q < c->npairs; ++q) cps[pc[q] + 1]++;
+  for (int e = 0; e < ncell; ++e) cps[e + 1] += cps[e];
+  {
+    std::vector<int> fill(cps.begin(), cps.end() - 1);
+    for (long q = 0; q < c->npairs; ++q) cpi[fill[pc[q]]++] = (int)q;
+  }
+  // K-extension entries: every cell sharing a node with a pair cell of the atom (the pair cells and their 26 neighbours)
+  std::vector<std::vector<int>> cell_atoms(ncell);
+  for (int a = 0; a < natoms; ++a) {
+    std::set<int> cells;
+    for (int q = c->h_atom_pair_start[a]; q < c->h_atom_pair_start[a + 1]; ++q) {
+      int cx, cy, cz;
+      mesh_cell_coords(c->md, pc[q], &cx, &cy, &cz);
+      for (int dx = -1; dx <= 1; ++dx)
+        for (int dy = -1; dy <= 1; ++dy)
+          for (int dz = -1; dz <= 1; ++dz) {
+            int x = cx + dx, y = cy + dy, z = cz + dz;
+            if (per) { x = (x + c->nc[0]) % c->nc[0]; y = (y + c->nc[1]) % c->nc[1]; z = (z + c->nc[2]) % c->nc[2]; }
+            else if (x < 0 || y < 0 || z < 0 || x >= c->nc[0] || y >= c->nc[1] || z >= c->nc[2]) continue;
+            cells.insert((x * c->nc[1] + y) * c->nc[2] + z);
+          }
+    }
+    for (int e : cells) cell_atoms[e].push_back(a);
+  }
+  std::vector<int> es(ncell + 1, 0), ea, ec;
+  for (int e = 0; e < ncell; ++e) {
+    for (int a : cell_atoms[e]) { ea.push_back(a); ec.push_back(e); }
+    es[e + 1] = (int)ea.size();
+  }
+  p->nchunks = (long)ea.size();
+  // neighbour atoms: b in nb(a) iff some pair cell of a is an extension cell of b
+  std::vector<std::set<int>> nbs(natoms);
+  for (int e = 0; e < ncell; ++e)
+    for (int q = cps[e]; q < cps[e + 1]; ++q)
+      for (int b : cell_atoms[e]) nbs[pa[cpi[q]]].insert(b);
+  std::vector<int> ns(natoms + 1, 0), na;
+  for (int a = 0; a < natoms; ++a) { for (int b : nbs[a]) na.push_back(b); ns[a + 1] = (int)na.size(); }
+  const long nnb = (long)na.size();
+  p->ext_ksteps = (2 * npj + 7) / 8;
+  if (p->nchunks == 0) { p->ok = true; return PAWFE_OK; }
+
+  int *d_ec = nullptr, *d_cps = nullptr, *d_cpi = nullptr;
+  double* d_G = nullptr;
+  pawfe_status st = PAWFE_OK;
+  auto cleanup = [&]() { cudaFree(d_ec); cudaFree(d_cps); cudaFree(d_cpi); cudaFree(d_G); };
+#define TRYP(xx) do { st = (xx); if (st != PAWFE_OK) { cleanup(); return st; } } while (0)
+  TRYP(upload(c, &p->d_ext_start, es)); TRYP(upload(c, &p->d_ext_atom, ea)); TRYP(upload(c, &d_ec, ec));
+  TRYP(upload(c, &d_cps, cps)); TRYP(upload(c, &d_cpi, cpi));
+  TRYP(upload(c, &p->d_nb_start, ns)); TRYP(upload(c, &p->d_nb_atom, na));
+  TRYP(dev_alloc(c, &p->d_Bext, (size_t)p->nchunks * n * 32));
+  TRYP(dev_alloc(c, &d_G, (size_t)nnb * npj * npj));
+  cudaMemsetAsync(d_G, 0, (size_t)nnb * npj * npj * sizeof(double), c->stream);
+  size_t smem = (size_t)n * npj * sizeof(double);
+  cudaError_t e = cudaFuncSetAttribute(k_build_ext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) {
+    k_build_ext<<<(unsigned)p->nchunks, 256, smem, c->stream>>>(
+        c->md, d_ec, p->d_ext_atom, c->d_atom_pair_start, c->d_pair_cell, (const double*)c->d_Cd64, npj,
+        (const double*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, p->d_Bext, d_G);
+    c->launches++;
+    e = cudaGetLastError();
+  }
+  std::vector<double> G((size_t)nnb * npj * npj);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess) e = cudaMemcpy(G.data(), d_G, G.size() * sizeof(double), cudaMemcpyDeviceToHost);
+  cleanup();
+  if (e != cudaSuccess) { c->err = std::string("fused plan build: ") + cudaGetErrorString(e); return PAWFE_ECUDA; }
+#undef TRYP
+  // GD^{ab} = G^{ab} Delta^b_Sinv; cross-check the diagonal blocks against G^a of atoms_create
+  std::vector<float> GD((size_t)nnb * npj * npj);
+  const size_t per2 = (size_t)npj * npj;
+  for (int a = 0; a < natoms; ++a)
+    for (int s = ns[a]; s < ns[a + 1]; ++s) {
+      const int b = na[s];
+      const double* g = &G[(size_t)s * per2];
+      if (b == a) {
+        double dmax = 0, gmax = 0;
+        for (size_t i = 0; i < per2; ++i) { dmax = std::max(dmax, std::fabs(g[i] - c->h_G[a * per2 + i])); gmax = std::max(gmax, std::fabs(g[i])); }
+        if (dmax > 1e-9 * std::max(gmax, 1e-300)) { c->err = "fused plan: G^{aa} from the extension blocks disagrees with atoms_create"; return PAWFE_ECUDA; }
+      }
+      const double* si = &c->h_dSinv[(size_t)b * per2];
+      for (int i = 0; i < npj; ++i)
+        for (int j = 0; j < npj; ++j) {
+          double t = 0;
+          for (int k = 0; k < npj; ++k) t += g[i * npj + k] * si[k * npj + j];
+          GD[(size_t)s * per2 + i * npj + j] = (float)t;
+        }
+    }
+  TRY(upload(c, &p->d_GD, GD));
+  p->ok = true;
+  return PAWFE_OK;
+}
+
+pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int B) {
+  if (B <= p->Bcap) return PAWFE_OK;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  cudaFree(p->d_P1); cudaFree(p->d_Wcat); p->d_P1 = p->d_Wcat = nullptr; p->Bcap = 0;
+  const long ldw = roundup4(B);
+  const size_t na = (size_t)std::max(1, c->natoms);
+  TRY(dev_alloc(c, &p->d_P1, na * c->npj * ldw));
+  TRY(dev_alloc(c, &p->d_Wcat, na * 32 * ldw));
+  CUDA_TRY(c, cudaMemsetAsync(p->d_Wcat, 0, na * 32 * ldw * sizeof(float), c->stream));
+  p->Bcap = B; p->ldw = ldw;
+  return PAWFE_OK;
+}
+
+// P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple)
+pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
+  if (c->npairs == 0) return PAWFE_OK;
+  const int n = c->n, npj = c->npj;
+  CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
+  size_t smem = (size_t)n * 8 + (size_t)npj * n * 4 + 16 * 128 * 4;
+  static size_t smem_attr = 0;
+  if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+  k_proj2<<<dim3((unsigned)c->npairs, ceil_div(B, 128)), 256, smem, c->stream>>>(
+      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, npj, X, ldx, B, p->d_P1, p->ldw);
+  KERNEL_CHECK(c, "k_proj2");
+  k_couple<<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
+      npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
+      p->d_GD, p->d_Wcat, p->ldw);
+  KERNEL_CHECK(c, "k_couple");
+  return PAWFE_OK;
+}
+
+TcExt make_ext(const FusedPlan* p, int scale_mode) {
+  TcExt x;
+  x.scale_mode = scale_mode; x.nchunks = p->nchunks; x.ext_start = p->d_ext_start; x.ext_atom = p->d_ext_atom;
+  x.Bext = p->d_Bext; x.Wcat = p->d_Wcat; x.ldw = p->ldw; x.ksteps = p->ext_ksteps;
+  return x;
+}
+
+}  // namespace
+
+void fused_invalidate(pawfe_ctx* c) {
+  if (c->fused) { free_plan((FusedPlan*)c->fused); c->fused = nullptr; }
+}
+
+bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
+  return prec == PAWFE_TF32 && !c->cplx && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
+}
+
+pawfe_status fused_prepare(pawfe_ctx* c, int B) {
+  FusedPlan* p = (FusedPlan*)c->fused;
+  if (!p) {
+    p = new FusedPlan();
+    c->fused = p;
+    pawfe_status st = build_plan(c, p);
+    if (st != PAWFE_OK) { fused_invalidate(c); return st; }
+  }
+  return ensure_scratch(c, p, B);
+}
+
+pawfe_status fused_apply_H(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B) {
+  TRY(fused_prepare(c, B));
+  FusedPlan* p = (FusedPlan*)c->fused;
+  TRY(project_and_couple(c, p, X, ldx, B, 2));
+  if (ldy == B) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * B * sizeof(float), c->stream));
+  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)B * sizeof(float), c->M, c->stream));
+  TcExt x = make_ext(p, 0);
+  prof_begin(c);
+  pawfe_status st = tc_cell_apply(c, X, ldx, Y, ldy, B, 1.0f, &x);
+  prof_end(c);
+  return st;
+}
+
+pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const double* as, const double* acs,
+                               const double* zzs, double z_over_e, float* X, long ld, int B, void* workspace) {
+  TRY(fused_prepare(c, B));
+  FusedPlan* p = (FusedPlan*)c->fused;
+  // workspace arrays use this block's own padded leading dimension; P1 / Wcat use the plan's (widest block seen)
+  const long ldw = roundup4(B);
+  const size_t blk_s = ((size_t)c->M * ldw * 4 + 255) / 256 * 256, blk_d = ((size_t)c->M * ldw * 8 + 255) / 256 * 256;
+  char* ws = (char*)workspace;
+  double* Yt = (double*)ws;
+  double* SX = (double*)(ws + blk_d);
+  float* RX = (float*)(ws + 2 * blk_d);
+  float* RY = (float*)(ws + 2 * blk_d + blk_s);
+  // ---- step 2 (FP64): H X and S X ----
+  TRY((pawfe_apply_HS<float, double, double>(c, 0, false, X, ld, Yt, ldw, B)));
+  TRY((pawfe_apply_HS<float, double, double>(c, 1, false, X, ld, SX, ldw, B)));
+  const int gs = 8 * c->sm_count;
+  k_residual_init2<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, SX, ds, z_over_e, RX, RY);
+  KERNEL_CHECK(c, "k_residual_init2");
+  // ---- step 4 ----
+  TcExt x = make_ext(p, 1);
+  const long nquads = c->M * (ldw / 4);
+  for (int th = 2; th <= m; ++th) {
+    TRY(project_and_couple(c, p, RY, ldw, B, 0));
+    k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
+                                         ds + (size_t)(th - 1) * B, B, (float)acs[th], (float)zzs[th]);
+    KERNEL_CHECK(c, "k_prepass");
+    prof_begin(c);
+    pawfe_status st = tc_cell_apply(c, RY, ldw, RX, ldw, B, (float)as[th], &x);
+    prof_end(c);
+    TRY(st);
+    std::swap(RX, RY);
+  }
+  // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----
+  TRY(project_and_couple(c, p, RY, ldw, B, 1));
+  k_recover2<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, RY, X, ld, ds + (size_t)m * B);
+  KERNEL_CHECK(c, "k_recover2");
+  if (c->npairs > 0) {
+    size_t smem = (size_t)c->n * 12 + (size_t)c->npj * c->n * 4;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatter2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_scatter2<<<dim3((unsigned)c->npairs, ceil_div(B, 128)), 256, smem, c->stream>>>(
+        c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, c->npj, p->d_Wcat, p->ldw, B, -1.0f, X, ld);
+    KERNEL_CHECK(c, "k_scatter2");
+  }
+  return PAWFE_OK;
+}

@@ -38,23 +38,29 @@ struct TcArgs {
   int B; float alpha;
   int n, NH, NT, kchunks, ksteps_last, nvt, ntiles;
   uint32_t tmem_cols, idesc;
+  int scale_mode;            // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
+  // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
+  const int* ext_start; const int* ext_atom; const float* Wcat; long ldw; int ext_ksteps;
   int dbg;
 };
 
 struct TcPlan {
   CUtensorMap tmapH;
+  CUtensorMap tmapE;             // K-extension blocks [chunk * n + I][32], built on first use for ext_ptr
+  const void* ext_ptr = nullptr;
   int NT = 0, NH = 0;
   bool ok = false;
 };
 
 __global__ void __launch_bounds__(kThreads, 2)
-k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
+k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant__ CUtensorMap tmapE, const TcArgs a) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const int bbytes = a.NT * 128;
   uint8_t* sA = smem;                                  // [kStages][16 KB]
   uint8_t* sB = smem + kStages * kABytes;              // [kStages][NT * 128 B]
   long* nodeJ = reinterpret_cast<long*>(sB + kStages * bbytes);          // [NH * NT] global row or -1
-  uint64_t* full = reinterpret_cast<uint64_t*>(nodeJ + a.NH * a.NT);      // [kStages]
+  float* nodeS = reinterpret_cast<float*>(nodeJ + a.NH * a.NT);          // [NH * NT] output scale per node
+  uint64_t* full = reinterpret_cast<uint64_t*>(nodeS + a.NH * a.NT);      // [kStages]
   uint64_t* empty = full + kStages;                                       // [kStages]
   uint64_t* accum = empty + kStages;                                      // [1]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
@@ -65,7 +71,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
     ptx::mbar_init(accum, 1);
     ptx::fence_barrier_init();
   }
-  if (warp == 4 && lane == 0) ptx::prefetch_tmap(&tmapH);
+  if (warp == 4 && lane == 0) { ptx::prefetch_tmap(&tmapH); if (a.ext_start) ptx::prefetch_tmap(&tmapE); }
   if (warp == 5) ptx::tmem_alloc(tmem_slot, a.tmem_cols);
   ptx::tc_fence_before_sync();
   __syncthreads();
@@ -81,6 +87,8 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
     const int rem = tile - cell * per_cell;
     const int vt = rem / a.NH, half = rem - vt * a.NH;
     const int v0 = vt * kTileV;
+    const int ext0 = a.ext_start ? a.ext_start[cell] : 0;
+    const int nchunks = a.kchunks + (a.ext_start ? a.ext_start[cell + 1] - ext0 : 0);
 
     __syncthreads();  // previous tile's readers of nodeJ are done
     {
@@ -88,13 +96,17 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
       mesh_cell_coords(a.md, cell, &cx, &cy, &cz);
       for (int I = threadIdx.x; I < a.NH * a.NT; I += kThreads) {
         long J = -1;
+        float sc = 0.f;
         if (I < a.n) {
           int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1);
           int ix, iy, iz;
           J = mesh_node(a.md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-          if (a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz] == 0.0) J = -1;  // Dirichlet boundary
+          const double mi = a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz];
+          if (mi == 0.0) J = -1;  // Dirichlet boundary
+          sc = a.scale_mode ? (float)((double)a.alpha * mi) : a.alpha;
         }
         nodeJ[I] = J;
+        nodeS[I] = sc;
       }
     }
     __syncthreads();
@@ -102,19 +114,28 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
     if (warp < 4) {
       // ================= gather producers: X rows -> swizzled MN-major A tiles =================
       const int t = threadIdx.x;  // 0..127
-      for (int c = 0; c < a.kchunks; ++c) {
+      for (int c = 0; c < nchunks; ++c) {
         const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
         ptx::mbar_wait(&empty[s], ph ^ 1);
         const uint32_t abase = ptx::smem_u32(sA + s * kABytes);
+        const bool isext = c >= a.kchunks;
+        const float* wrows = isext ? a.Wcat + (long)a.ext_atom[ext0 + c - a.kchunks] * 32 * a.ldw : nullptr;
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const int op = i * 128 + t;
           const int row = op >> 5, c16all = op & 31;   // one warp covers one 512-byte row
           const int k = c * kChunkK + row;
           const int v = v0 + c16all * 4;
-          long J = (k < a.n) ? nodeJ[k] : -1;
-          const bool ok = (J >= 0) && (v < a.B);
-          const float* src = ok ? (a.X + J * a.ldx + v) : a.X;
+          const float* src;
+          bool ok;
+          if (!isext) {
+            long J = (k < a.n) ? nodeJ[k] : -1;
+            ok = (J >= 0) && (v < a.B);
+            src = ok ? (a.X + J * a.ldx + v) : a.X;
+          } else {
+            ok = v < a.B;
+            src = ok ? (wrows + (long)row * a.ldw + v) : a.X;
+          }
           // MN-major tf32 layout (128-byte swizzle, 32-byte atoms): 32-vector column block cb at cb * 4096;
           // row r at r * 128; its four 32-byte chunks q stored at q ^ (r % 4)
           const uint32_t dst = abase + (c16all >> 3) * 4096 + row * 128 +
@@ -130,7 +151,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
       }
       ptx::cp_async_wait<0>();
       ptx::fence_proxy_async_smem();
-      ptx::mbar_arrive(&full[(it + a.kchunks - 1) % kStages]);
+      ptx::mbar_arrive(&full[(it + nchunks - 1) % kStages]);
 
       // ================= epilogue: TMEM -> scaled atomic adds into Y (assembly) =================
       ptx::mbar_wait(accum, tile_iter & 1);
@@ -150,29 +171,32 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
           const long J = nodeJ[half * a.NT + col0 + j];
-          if (J >= 0 && vok) atomicAdd(a.Y + J * a.ldy + v, a.alpha * __uint_as_float(r[j]));
+          if (J >= 0 && vok) atomicAdd(a.Y + J * a.ldy + v, nodeS[half * a.NT + col0 + j] * __uint_as_float(r[j]));
         }
       }
       ptx::tc_fence_before_sync();
     } else if (warp == 4) {
       // ================= TMA producer: H^e row block, one K chunk per stage =================
       if (lane == 0) {
-        for (int c = 0; c < a.kchunks; ++c) {
+        for (int c = 0; c < nchunks; ++c) {
           const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
           ptx::mbar_wait(&empty[s], ph ^ 1);
           ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
-          ptx::tma_load_2d(ptx::smem_u32(sB + s * bbytes), &tmapH, c * kChunkK, cell * a.n + half * a.NT, &full[s]);
+          if (c < a.kchunks)
+            ptx::tma_load_2d(ptx::smem_u32(sB + s * bbytes), &tmapH, c * kChunkK, cell * a.n + half * a.NT, &full[s]);
+          else
+            ptx::tma_load_2d(ptx::smem_u32(sB + s * bbytes), &tmapE, 0, (ext0 + c - a.kchunks) * a.n + half * a.NT, &full[s]);
         }
       }
     } else {
       // ================= MMA issuer =================
       if (lane == 0) {
-        for (int c = 0; c < a.kchunks; ++c) {
+        for (int c = 0; c < nchunks; ++c) {
           const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
           ptx::mbar_wait(&full[s], ph);
           ptx::tc_fence_after_sync();
           const uint32_t abase = ptx::smem_u32(sA + s * kABytes), bbase = ptx::smem_u32(sB + s * bbytes);
-          const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : kChunkK / 8;
+          const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
 #ifdef PAWFE_TC_DEBUG
           if (blockIdx.x == 0 && c == 0) {
             const float* Af = reinterpret_cast<const float*>(sA + s * kABytes);
@@ -199,7 +223,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const TcArgs a) {
       }
       __syncwarp();
     }
-    it += a.kchunks;
+    it += nchunks;
   }
   __syncthreads();
   if (warp == 5) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
@@ -228,7 +252,7 @@ void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
 }
 
 size_t smem_bytes(int NH, int NT) {
-  return (size_t)kStages * (kABytes + NT * 128) + (size_t)NH * NT * 8 + (2 * kStages + 1) * 8 + 16;
+  return (size_t)kStages * (kABytes + NT * 128) + (size_t)NH * NT * 12 + (2 * kStages + 1) * 8 + 16;
 }
 
 TcPlan* get_plan(pawfe_ctx* c) {
@@ -278,7 +302,8 @@ bool tc_usable(pawfe_ctx* c, const void* X, long ldx, const void* Y, long ldy, i
   return get_plan(c)->ok;
 }
 
-pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B, float alpha) {
+pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B, float alpha,
+                           const TcExt* ext) {
   TcPlan* p = get_plan(c);
   if (!p->ok) { c->err = "tcgen05 cell kernel: tensor map / attribute set-up failed"; return PAWFE_EUNSUPPORTED; }
   TcArgs a;
@@ -292,13 +317,34 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   while ((int)cols < a.NT) cols <<= 1;
   a.tmem_cols = cols;
   a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
+  a.scale_mode = 0;
+  a.ext_start = nullptr; a.ext_atom = nullptr; a.Wcat = nullptr; a.ldw = 0; a.ext_ksteps = 0;
+  if (ext) {
+    a.scale_mode = ext->scale_mode;
+    if (ext->nchunks > 0) {
+      if (p->ext_ptr != ext->Bext) {
+        EncodeTiledFn enc = get_encode();
+        cuuint64_t dims[2] = {32, (cuuint64_t)ext->nchunks * c->n};
+        cuuint64_t strides[1] = {32 * sizeof(float)};
+        cuuint32_t box[2] = {(cuuint32_t)kChunkK, (cuuint32_t)p->NT};
+        cuuint32_t estr[2] = {1, 1};
+        CUresult r = enc(&p->tmapE, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)ext->Bext, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { c->err = "tcgen05 cell kernel: K-extension tensor map failed"; return PAWFE_ECUDA; }
+        p->ext_ptr = ext->Bext;
+      }
+      a.ext_start = ext->ext_start; a.ext_atom = ext->ext_atom; a.Wcat = ext->Wcat; a.ldw = ext->ldw;
+      a.ext_ksteps = ext->ksteps;
+    }
+  }
   a.dbg = 0;
 #ifdef PAWFE_TC_DEBUG
   a.dbg = getenv("PAWFE_TC_DBG") ? atoi(getenv("PAWFE_TC_DBG")) : 0;
   if (a.dbg & 1) a.idesc = ptx::idesc_tf32(kTileV, a.NT, 0, 0);
 #endif
   int grid = std::min(a.ntiles, 2 * c->sm_count);
-  k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT), c->stream>>>(p->tmapH, a);
+  k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT), c->stream>>>(p->tmapH, a.ext_start ? p->tmapE : p->tmapH, a);
   KERNEL_CHECK(c, "k_cell_tcgen05");
   return PAWFE_OK;
 }

@@ -13,6 +13,21 @@ bool tc_supported(const pawfe_ctx* ctx, int B);
 // dimensions and B multiples of 4) and the tensor map could be built.
 bool tc_usable(pawfe_ctx* ctx, const void* X, long ldx, const void* Y, long ldy, int B);
 
-// Y += alpha * sum_e P_e^T H^e (P_e X) for a real FP32 block, TF32 multiply, FP32 accumulate.
-// X, Y: device [dof][vec] float, leading dimensions ldx, ldy.  Y must already hold the values to add to.
-pawfe_status tc_cell_apply(pawfe_ctx* ctx, const float* X, long ldx, float* Y, long ldy, int B, float alpha);
+// Optional K-extension of the contraction (fused.h): cell e gets, after its own n input rows, one 32-row chunk
+// per listed (cell, atom) entry x in [ext_start[e], ext_start[e+1]): input rows Wcat[ext_atom[x]][0..32)[vec],
+// matrix block Bext[x][I][0..32) (I = output node).  This adds the low-rank projector terms to the product
+// inside the same MMA accumulation.  ksteps = ceil(used rows / 8).
+struct TcExt {
+  int scale_mode;              // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
+  long nchunks;
+  const int* ext_start; const int* ext_atom;
+  const float* Bext;
+  const float* Wcat; long ldw;
+  int ksteps;
+};
+
+// Y += alpha * [M_D^-1] sum_e P_e^T (H^e (P_e X) + extension terms) for a real FP32 block, TF32 multiply, FP32
+// accumulate.  X, Y: device [dof][vec] float, leading dimensions ldx, ldy.  Y must already hold the values to
+// add to (assembly is by atomic adds).  ext may be null.
+pawfe_status tc_cell_apply(pawfe_ctx* ctx, const float* X, long ldx, float* Y, long ldy, int B, float alpha,
+                           const TcExt* ext = nullptr);

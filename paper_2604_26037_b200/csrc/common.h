@@ -165,6 +165,7 @@ struct pawfe_ctx {
   void* d_Cd32 = nullptr;  // same, float / float2
   std::vector<double> h_dS;          // natoms*npj*npj real
   std::vector<double> h_G;           // natoms*npj*npj scalars: G^a = C^a^dagger M_D^-1 C^a
+  std::vector<double> h_dSinv;       // natoms*npj*npj scalars: Delta^a_Sinv (Eq. 29)
   void* d_D64 = nullptr; void* d_dS64 = nullptr; void* d_dSinv64 = nullptr;  // [atom][npj][npj] scalar
   void* d_D32 = nullptr; void* d_dS32 = nullptr; void* d_dSinv32 = nullptr;
   void* d_P = nullptr;   // projection scratch: 2 x [natoms][npj][512] scalar (FP64-complex sized)
@@ -179,6 +180,7 @@ struct pawfe_ctx {
   int scal_next = 0;
 
   void* tc_plan = nullptr;  // cell_tcgen05.cu: cached tensor map and tile shape
+  void* fused = nullptr;    // api_fused.cu: FusedPlan (K-extension blocks, neighbour couplings, scratch)
 
   // optional CUDA-event timing of the cell-contraction launches of the filter loop (pawfe_cell_timing)
   bool prof_on = false;

@@ -1,0 +1,33 @@
+// fused.h -- the fused Chebyshev step of Algorithm 2 for real FP32-storage blocks.
+//
+// One step  R_X <- a H S^-1approx R_Y - a c R_Y - zeta zeta1 R_X + a Y Lambda_Y  is computed without ever
+// writing T = S^-1approx R_Y or H T to memory:
+//   * the recurrence state is kept as  Rt = M_D^-1 R  (and Yt = M_D^-1 Y), so that T = Rt - M_D^-1 C W with
+//     W^a = Delta^a_Sinv C^a^dagger Rt  (Eq. 28) needs no diagonal scaling at gather time;
+//   * the low-rank terms are folded into the cell contraction as extra K rows ("K-extension"): for every
+//     (cell e, atom b) whose assembled projector support touches e,
+//         Y_e += [ -H^e (M_D^-1 C^b)|_e ,  C^{e,b} ] [ W^b ; D^b P2^b ],
+//     with P2^b = C^b^dagger T = P1^b - sum_a G^{ba} W^a,  G^{ba} = C^b^dagger M_D^-1 C^a  (exact algebra);
+//   * the bracket  -a c Rt_Y - zeta zeta1 Rt_X + a Yt Lambda_Y (FP64 add, L374)  is written first ("prepass") and the
+//     cell kernel's assembly adds  a M_D^-1 H T  on top of it with atomic adds.
+#pragma once
+#include "common.h"
+
+struct FusedPlan;
+
+// Build (on first use) the K-extension blocks, the neighbour couplings G^{ab} Delta^b_Sinv and scratch for block
+// width B.  Needs mesh, FP64 cell matrices and atoms.  Synchronises the stream the first time.
+pawfe_status fused_prepare(pawfe_ctx* c, int B);
+// Drop the plan (cell matrices or atoms changed).
+void fused_invalidate(pawfe_ctx* c);
+// The couplings D changed: nothing to rebuild (D is read at run time), kept for symmetry.
+bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B);
+
+// Algorithm 2 for a real context in FP32 storage with the TF32 tcgen05 contraction.  Coefficients come from
+// pawfe_filter_scalars (api_filter.cu).  X: [dof][vec] float, ld >= B.  workspace as pawfe_filter_workspace.
+pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds /*device scalars*/, const double* as,
+                               const double* acs, const double* zzs, double z_over_e, float* X, long ld, int B,
+                               void* workspace);
+
+// Y = H X (TF32 contraction, non-local term through the K-extension).  X, Y float, 16-byte aligned, ld % 4 == 0.
+pawfe_status fused_apply_H(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B);

@@ -5,6 +5,7 @@
 #include "common.h"
 #include "fe_tables.h"
 #include "host_util.h"
+#include "fused.h"
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -22,8 +23,10 @@ void pawfe_free_pot(pawfe_ctx* c) {
   cudaFree(c->d_H32); c->d_H32 = nullptr;
   c->have_pot = false; c->have_h64 = false;
   tc_invalidate(c);
+  fused_invalidate(c);
 }
 void pawfe_free_atoms(pawfe_ctx* c) {
+  fused_invalidate(c);
   cudaFree(c->d_pair_cell); cudaFree(c->d_pair_atom); cudaFree(c->d_atom_pair_start);
   cudaFree(c->d_Cd64); cudaFree(c->d_Cd32);
   cudaFree(c->d_D64); cudaFree(c->d_dS64); cudaFree(c->d_dSinv64);
