@@ -5,6 +5,7 @@
 #include "host_util.h"
 #include "kernels_simt.cuh"
 #include "kernels_stream.cuh"
+#include "cell_dmma.cuh"
 #include "api_internal.h"
 #include "apply_impl.h"
 #include "fused.h"
@@ -57,9 +58,43 @@ pawfe_status zero_block(pawfe_ctx* c, TY* Y, long ldy, int B) {
   return PAWFE_OK;
 }
 
+// FP64 cell product on the DMMA pipe (cell_dmma.cuh).  RX: real type of the input block.
+template <typename RX, bool CPLX, int MT>
+pawfe_status launch_dmma_mt(pawfe_ctx* c, const double* A, long cell_stride, const RX* X, long ldx, double* Y, long ldy,
+                            int Wr, double alpha) {
+  auto kern = dmma::k_cell_dmma<RX, CPLX, MT>;
+  const size_t smem = dmma::smem_bytes<RX, CPLX, MT>(c->n);
+  static size_t smem_attr = 0;
+  if (smem > smem_attr) {
+    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    smem_attr = smem;
+  }
+  kern<<<dim3(c->ncell, ceil_div(Wr, dmma::kTN)), dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  KERNEL_CHECK(c, "k_cell_dmma");
+  return PAWFE_OK;
+}
+template <typename RX, bool CPLX>
+pawfe_status launch_dmma(pawfe_ctx* c, const double* A, long cell_stride, const RX* X, long ldx, double* Y, long ldy,
+                         int Wr, double alpha) {
+  const int n = c->n;
+  if (n <= 32) return launch_dmma_mt<RX, CPLX, 1>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  if (n <= 64) return launch_dmma_mt<RX, CPLX, 2>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  if (n <= 128) return launch_dmma_mt<RX, CPLX, 4>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  if (n <= 224) return launch_dmma_mt<RX, CPLX, 7>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  if (n <= 352) return launch_dmma_mt<RX, CPLX, 11>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  return launch_dmma_mt<RX, CPLX, 8>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+}
+
 template <typename TX, typename TY, typename TC, bool TF32>
 pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, const TX* X, long ldx, TY* Y,
                          long ldy, int B, int in_scale, double alpha) {
+  if constexpr (sizeof(typename ScalarTraits<TC>::real) == 8) {
+    // FP64 compute: DMMA kernel (lda == n, no input scaling on this path)
+    constexpr bool CP = ScalarTraits<TC>::cplx;
+    constexpr int cw = CP ? 2 : 1;
+    typedef typename ScalarTraits<TX>::real RX;
+    return launch_dmma<RX, CP>(c, (const double*)A, cell_stride, (const RX*)X, ldx * cw, (double*)Y, ldy * cw, B * cw, alpha);
+  } else {
   constexpr int BV = (sizeof(TC) == 16) ? 16 : 32;
   size_t smem = (size_t)c->n * 16 + (size_t)c->n * BV * sizeof(TC);
   auto kern = k_cell_simt<TX, TY, TC, BV, TF32>;
@@ -72,6 +107,7 @@ pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, c
                                                                   in_scale, alpha);
   KERNEL_CHECK(c, "k_cell_simt");
   return PAWFE_OK;
+  }
 }
 
 }  // namespace
