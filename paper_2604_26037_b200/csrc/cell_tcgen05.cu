@@ -25,23 +25,26 @@
 
 namespace {
 
-constexpr int kStages = 2;
 constexpr int kChunkK = 32;             // K rows per pipeline stage (= 128 bytes of a K-major tf32 row)
-constexpr int kTileV = 128;             // vectors per tile (MMA M)
-constexpr int kABytes = kChunkK * kTileV * 4;  // 16 KB
-constexpr int kThreads = 192;
+constexpr int kTileV = 128;             // vectors per MMA (M)
+constexpr int kABytes = kChunkK * kTileV * 4;  // 16 KB per vector tile and stage
+constexpr int kThreads = 320;           // warps 0-3 epilogue, 4-7 gather, 8 TMA, 9 MMA / TMEM owner
+constexpr int kMaxStages = 6;
 
 struct TcArgs {
   MeshDev md;
   const float* X; long ldx;
   float* Y; long ldy;
   int B; float alpha;
-  int n, NH, NT, kchunks, ksteps_last, nvt, ntiles;
+  int n, NH, NT, kchunks, ksteps_last;
+  int nvt;       // vector tiles of 128 in the block
+  int nvg;       // groups of up to 2 vector tiles (one CTA tile holds a group: both share every H^e load)
+  int ntiles;    // ncell * nvg * NH
+  int stages;
   uint32_t tmem_cols, idesc;
   int scale_mode;            // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
   // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
   const int* ext_start; const int* ext_atom; const float* Wcat; long ldw; int ext_ksteps;
-  int dbg;
 };
 
 struct TcPlan {
@@ -52,181 +55,208 @@ struct TcPlan {
   bool ok = false;
 };
 
-__global__ void __launch_bounds__(kThreads, 2)
+__device__ __forceinline__ void bar_sync_128(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+
+// Persistent CTAs (one per SM) loop over tiles (cell, vector group, node half).  Roles are decoupled across tiles:
+// the gather / TMA producers run ahead into the next tile through the shared-memory ring while the epilogue warps
+// drain the accumulators of the current one; the MMA issuer waits for the drained accumulator (accum_empty).
+__global__ void __launch_bounds__(kThreads, 1)
 k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant__ CUtensorMap tmapE, const TcArgs a) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const int bbytes = a.NT * 128;
-  uint8_t* sA = smem;                                  // [kStages][16 KB]
-  uint8_t* sB = smem + kStages * kABytes;              // [kStages][NT * 128 B]
-  long* nodeJ = reinterpret_cast<long*>(sB + kStages * bbytes);          // [NH * NT] global row or -1
-  float* nodeS = reinterpret_cast<float*>(nodeJ + a.NH * a.NT);          // [NH * NT] output scale per node
-  uint64_t* full = reinterpret_cast<uint64_t*>(nodeS + a.NH * a.NT);      // [kStages]
-  uint64_t* empty = full + kStages;                                       // [kStages]
-  uint64_t* accum = empty + kStages;                                      // [1]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum + 1);
+  const int abytes = 2 * kABytes;                       // room for two vector tiles
+  const int sbytes = abytes + bbytes;                   // one stage: [A vt0][A vt1][B]
+  long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows (-1: none)
+  long* eJ = gJ + a.NH * a.NT;                                            // [NT] output rows of this half
+  float* eS = reinterpret_cast<float*>(eJ + a.NT);                        // [NT] output scale
+  uint64_t* full = reinterpret_cast<uint64_t*>(eS + a.NT);                // [stages]
+  uint64_t* empty = full + kMaxStages;                                    // [stages]
+  uint64_t* accum_full = empty + kMaxStages;
+  uint64_t* accum_empty = accum_full + 1;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_empty + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { ptx::mbar_init(&full[s], 128 + 1); ptx::mbar_init(&empty[s], 1); }
-    ptx::mbar_init(accum, 1);
+    for (int s = 0; s < a.stages; ++s) { ptx::mbar_init(&full[s], 128 + 1); ptx::mbar_init(&empty[s], 1); }
+    ptx::mbar_init(accum_full, 1);
+    ptx::mbar_init(accum_empty, 128);
     ptx::fence_barrier_init();
   }
-  if (warp == 4 && lane == 0) { ptx::prefetch_tmap(&tmapH); if (a.ext_start) ptx::prefetch_tmap(&tmapE); }
-  if (warp == 5) ptx::tmem_alloc(tmem_slot, a.tmem_cols);
+  if (warp == 8 && lane == 0) { ptx::prefetch_tmap(&tmapH); if (a.ext_start) ptx::prefetch_tmap(&tmapE); }
+  if (warp == 9) ptx::tmem_alloc(tmem_slot, a.tmem_cols);
   ptx::tc_fence_before_sync();
   __syncthreads();
   ptx::tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
+  const int n1 = a.md.n1;
+  const int per_cell = a.nvg * a.NH;
 
   uint32_t it = 0;        // running chunk counter (same sequence in every role)
   uint32_t tile_iter = 0;
-  const int n1 = a.md.n1;
   for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++tile_iter) {
-    const int per_cell = a.nvt * a.NH;
     const int cell = tile / per_cell;
     const int rem = tile - cell * per_cell;
-    const int vt = rem / a.NH, half = rem - vt * a.NH;
-    const int v0 = vt * kTileV;
+    const int vg = rem / a.NH, half = rem - vg * a.NH;
+    const int v0 = vg * 2 * kTileV;
+    const int nv = min(2, a.nvt - 2 * vg);            // vector tiles in this group
     const int ext0 = a.ext_start ? a.ext_start[cell] : 0;
     const int nchunks = a.kchunks + (a.ext_start ? a.ext_start[cell + 1] - ext0 : 0);
-
-    __syncthreads();  // previous tile's readers of nodeJ are done
-    {
-      int cx, cy, cz;
-      mesh_cell_coords(a.md, cell, &cx, &cy, &cz);
-      for (int I = threadIdx.x; I < a.NH * a.NT; I += kThreads) {
-        long J = -1;
-        float sc = 0.f;
-        if (I < a.n) {
-          int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1);
-          int ix, iy, iz;
-          J = mesh_node(a.md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-          const double mi = a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz];
-          if (mi == 0.0) J = -1;  // Dirichlet boundary
-          sc = a.scale_mode ? (float)((double)a.alpha * mi) : a.alpha;
-        }
-        nodeJ[I] = J;
-        nodeS[I] = sc;
-      }
-    }
-    __syncthreads();
+    int cx, cy, cz;
+    mesh_cell_coords(a.md, cell, &cx, &cy, &cz);
 
     if (warp < 4) {
-      // ================= gather producers: X rows -> swizzled MN-major A tiles =================
-      const int t = threadIdx.x;  // 0..127
-      for (int c = 0; c < nchunks; ++c) {
-        const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
-        ptx::mbar_wait(&empty[s], ph ^ 1);
-        const uint32_t abase = ptx::smem_u32(sA + s * kABytes);
-        const bool isext = c >= a.kchunks;
-        const float* wrows = isext ? a.Wcat + (long)a.ext_atom[ext0 + c - a.kchunks] * 32 * a.ldw : nullptr;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const int op = i * 128 + t;
-          const int row = op >> 5, c16all = op & 31;   // one warp covers one 512-byte row
-          const int k = c * kChunkK + row;
-          const int v = v0 + c16all * 4;
-          const float* src;
-          bool ok;
-          if (!isext) {
-            long J = (k < a.n) ? nodeJ[k] : -1;
-            ok = (J >= 0) && (v < a.B);
-            src = ok ? (a.X + J * a.ldx + v) : a.X;
-          } else {
-            ok = v < a.B;
-            src = ok ? (wrows + (long)row * a.ldw + v) : a.X;
-          }
-          // MN-major tf32 layout (128-byte swizzle, 32-byte atoms): 32-vector column block cb at cb * 4096;
-          // row r at r * 128; its four 32-byte chunks q stored at q ^ (r % 4)
-          const uint32_t dst = abase + (c16all >> 3) * 4096 + row * 128 +
-                               (((((c16all & 7) >> 1) ^ (row & 3)) << 5) | ((c16all & 1) << 4));
-          ptx::cp_async16(dst, src, ok ? 16u : 0u);
+      // ================= epilogue: TMEM -> scaled atomic adds into Y (assembly, Fig. 2 step iv) =================
+      bar_sync_128(2);   // previous tile's readers of eJ / eS are done
+      for (int I = threadIdx.x; I < a.NT; I += 128) {
+        const int Ig = half * a.NT + I;
+        long J = -1;
+        float sc = 0.f;
+        if (Ig < a.n) {
+          int c = Ig % n1, b = (Ig / n1) % n1, aa = Ig / (n1 * n1), ix, iy, iz;
+          J = mesh_node(a.md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+          const double mi = a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz];
+          J = (mi == 0.0) ? -1 : J * a.ldy * 4;  // byte offset of the output row; -1: Dirichlet boundary
+          sc = a.scale_mode ? (float)((double)a.alpha * mi) : a.alpha;
         }
-        ptx::cp_async_commit();
-        if (c >= 1) {
-          ptx::cp_async_wait<1>();
-          ptx::fence_proxy_async_smem();
-          ptx::mbar_arrive(&full[(it + c - 1) % kStages]);
-        }
+        eJ[I] = J; eS[I] = sc;
       }
-      ptx::cp_async_wait<0>();
-      ptx::fence_proxy_async_smem();
-      ptx::mbar_arrive(&full[(it + nchunks - 1) % kStages]);
-
-      // ================= epilogue: TMEM -> scaled atomic adds into Y (assembly) =================
-      ptx::mbar_wait(accum, tile_iter & 1);
+      bar_sync_128(2);
+      ptx::mbar_wait(accum_full, tile_iter & 1);
       ptx::tc_fence_after_sync();
-      const int v = v0 + warp * 32 + lane;
-      const bool vok = v < a.B;
-      for (int col0 = 0; col0 < a.NT; col0 += 16) {
-        if (half * a.NT + col0 >= a.n) break;
-        uint32_t r[16];
-        ptx::tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)col0, r);
-        ptx::tmem_ld_wait();
-#ifdef PAWFE_TC_DEBUG
-        if (blockIdx.x == 0 && threadIdx.x == 0 && col0 == 0)
-          printf("epi: tmem_base=%x r0=%g r1=%g r2=%g r15=%g J0=%ld v=%d vok=%d alpha=%g NT=%d n=%d\n", tmem_base, __uint_as_float(r[0]),
-                 __uint_as_float(r[1]), __uint_as_float(r[2]), __uint_as_float(r[15]), nodeJ[0], v, (int)vok, a.alpha, a.NT, a.n);
-#endif
+      const int ncols = min(a.NT, a.n - half * a.NT);
+      for (int j = 0; j < nv; ++j) {
+        const int v = v0 + j * kTileV + warp * 32 + lane;
+        const bool vok = v < a.B;
+        char* yv = reinterpret_cast<char*>(a.Y + v);
+        for (int col0 = 0; col0 < ncols; col0 += 32) {
+          uint32_t r[32];
+          const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(j * a.NT + col0);
+          ptx::tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(&r[0]));
+          if (col0 + 16 < ncols) ptx::tmem_ld16(taddr + 16, *reinterpret_cast<uint32_t(*)[16]>(&r[16]));
+          ptx::tmem_ld_wait();
+          if (vok) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const long J = nodeJ[half * a.NT + col0 + j];
-          if (J >= 0 && vok) atomicAdd(a.Y + J * a.ldy + v, nodeS[half * a.NT + col0 + j] * __uint_as_float(r[j]));
+            for (int q = 0; q < 32; q += 2) {
+              if (col0 + q < ncols) {   // ncols is even or the odd tail column has offset -1
+                const longlong2 off = *reinterpret_cast<const longlong2*>(&eJ[col0 + q]);
+                const float2 sc = *reinterpret_cast<const float2*>(&eS[col0 + q]);
+                if (off.x >= 0) atomicAdd(reinterpret_cast<float*>(yv + off.x), sc.x * __uint_as_float(r[q]));
+                if (off.y >= 0) atomicAdd(reinterpret_cast<float*>(yv + off.y), sc.y * __uint_as_float(r[q + 1]));
+              }
+            }
+          }
         }
       }
       ptx::tc_fence_before_sync();
-    } else if (warp == 4) {
-      // ================= TMA producer: H^e row block, one K chunk per stage =================
-      if (lane == 0) {
-        for (int c = 0; c < nchunks; ++c) {
-          const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
-          ptx::mbar_wait(&empty[s], ph ^ 1);
-          ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
-          if (c < a.kchunks)
-            ptx::tma_load_2d(ptx::smem_u32(sB + s * bbytes), &tmapH, c * kChunkK, cell * a.n + half * a.NT, &full[s]);
-          else
-            ptx::tma_load_2d(ptx::smem_u32(sB + s * bbytes), &tmapE, 0, (ext0 + c - a.kchunks) * a.n + half * a.NT, &full[s]);
+      ptx::mbar_arrive(accum_empty);
+    } else if (warp < 8) {
+      // ================= gather producers: X rows -> swizzled MN-major A tiles (Fig. 2 step i) =================
+      const int t = threadIdx.x - 128;  // 0..127
+      bar_sync_128(1);   // previous tile's readers of gJ are done
+      for (int I = t; I < a.NH * a.NT; I += 128) {
+        long J = -1;
+        if (I < a.n) {
+          int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+          J = mesh_node(a.md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+          J = (a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz] == 0.0) ? -1 : J * a.ldx * 4;  // byte offset
+        }
+        gJ[I] = J;
+      }
+      bar_sync_128(1);
+      // per-thread constants: this thread always copies 16-byte column lane of rows wg, wg + 4, ... of a chunk
+      const int wg = t >> 5;                               // row within each group of 4
+      const int vl = lane * 4;                             // first vector of the 16-byte piece inside the tile
+      // MN-major tf32 layout (128-byte swizzle, 32-byte atoms): 32-vector column block cb at cb * 4096; row r at
+      // r * 128; its four 32-byte chunks q stored at q ^ (r % 4); r % 4 == wg for every row this thread copies
+      const uint32_t dst_thread = (lane >> 3) * 4096 + wg * 128 + (((((lane & 7) >> 1) ^ wg) << 5) | ((lane & 1) << 4));
+      for (int c = 0; c < nchunks; ++c) {
+        const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
+        ptx::mbar_wait(&empty[s], ph ^ 1);
+        const uint32_t abase = ptx::smem_u32(smem + s * sbytes) + dst_thread;
+        if (c < a.kchunks) {
+          const long* offs = gJ + c * kChunkK + wg;
+          for (int j = 0; j < nv; ++j) {
+            const int v = v0 + j * kTileV + vl;
+            const bool vok = v < a.B;
+            const char* xv = reinterpret_cast<const char*>(a.X + v);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const long off = (c * kChunkK + wg + 4 * i < a.NH * a.NT) ? offs[4 * i] : -1;
+              const bool ok = vok && off >= 0;
+              ptx::cp_async16(abase + j * kABytes + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
+            }
+          }
+        } else {
+          const float* wrows = a.Wcat + ((long)a.ext_atom[ext0 + c - a.kchunks] * 32 + wg) * a.ldw;
+          for (int j = 0; j < nv; ++j) {
+            const int v = v0 + j * kTileV + vl;
+            const bool ok = v < a.B;
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              ptx::cp_async16(abase + j * kABytes + i * 512, ok ? wrows + (long)(4 * i) * a.ldw + v : a.X, ok ? 16u : 0u);
+          }
+        }
+        ptx::cp_async_commit();
+        if (c >= 2) {
+          ptx::cp_async_wait<2>();
+          ptx::fence_proxy_async_smem();
+          ptx::mbar_arrive(&full[(it + c - 2) % a.stages]);
         }
       }
+      if (nchunks >= 2) {
+        ptx::cp_async_wait<1>();
+        ptx::fence_proxy_async_smem();
+        ptx::mbar_arrive(&full[(it + nchunks - 2) % a.stages]);
+      }
+      ptx::cp_async_wait<0>();
+      ptx::fence_proxy_async_smem();
+      ptx::mbar_arrive(&full[(it + nchunks - 1) % a.stages]);
+    } else if (warp == 8) {
+      // ================= TMA producer: H^e row block (or K-extension block), one K chunk per stage =================
+      if (lane == 0) {
+        for (int c = 0; c < nchunks; ++c) {
+          const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
+          ptx::mbar_wait(&empty[s], ph ^ 1);
+          ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
+          const uint32_t dst = ptx::smem_u32(smem + s * sbytes + abytes);
+          if (c < a.kchunks)
+            ptx::tma_load_2d(dst, &tmapH, c * kChunkK, cell * a.n + half * a.NT, &full[s]);
+          else
+            ptx::tma_load_2d(dst, &tmapE, 0, (ext0 + c - a.kchunks) * a.n + half * a.NT, &full[s]);
+        }
+      }
+      __syncwarp();
     } else {
       // ================= MMA issuer =================
       if (lane == 0) {
+        ptx::mbar_wait(accum_empty, (tile_iter & 1) ^ 1);   // accumulators drained by the previous tile's epilogue
+        ptx::tc_fence_after_sync();
         for (int c = 0; c < nchunks; ++c) {
-          const uint32_t s = (it + c) % kStages, ph = ((it + c) / kStages) & 1;
+          const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
           ptx::mbar_wait(&full[s], ph);
           ptx::tc_fence_after_sync();
-          const uint32_t abase = ptx::smem_u32(sA + s * kABytes), bbase = ptx::smem_u32(sB + s * bbytes);
+          const uint32_t abase = ptx::smem_u32(smem + s * sbytes), bbase = abase + abytes;
           const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
-#ifdef PAWFE_TC_DEBUG
-          if (blockIdx.x == 0 && c == 0) {
-            const float* Af = reinterpret_cast<const float*>(sA + s * kABytes);
-            const float* Bf = reinterpret_cast<const float*>(sB + s * bbytes);
-            printf("mma: idesc=%x ksteps=%d kchunks=%d A[0]=%g A[1]=%g B[0]=%g B[1]=%g abase=%x bbase=%x\n", a.idesc, ksteps,
-                   a.kchunks, Af[0], Af[1], Bf[0], Bf[1], abase, bbase);
-          }
-#endif
           for (int ks = 0; ks < ksteps; ++ks) {
-            // A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
-            // 512 B apart (SBO); one K step = 8 rows = 1024 B
-            uint64_t adesc = ptx::smem_desc(abase + ks * 1024, 4096, 512, 1);
-#ifdef PAWFE_TC_DEBUG
-            if (a.dbg & 1) adesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);  // A := B tile, K-major
-            if (a.dbg & 2) adesc = ptx::smem_desc(abase + ks * 1024, 512, 4096, 1);  // swapped LBO/SBO
-#endif
             // B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B per K step inside the 128-B row
             const uint64_t bdesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);
-            ptx::mma_tf32_ss(tmem_base, adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+            for (int j = 0; j < nv; ++j) {
+              // A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
+              // 512 B apart (SBO); one K step = 8 rows = 1024 B
+              const uint64_t adesc = ptx::smem_desc(abase + j * kABytes + ks * 1024, 4096, 512, 1);
+              ptx::mma_tf32_ss(tmem_base + (uint32_t)(j * a.NT), adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+            }
           }
           ptx::mma_commit(&empty[s]);
         }
-        ptx::mma_commit(accum);
+        ptx::mma_commit(accum_full);
       }
       __syncwarp();
     }
     it += nchunks;
   }
   __syncthreads();
-  if (warp == 5) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
+  if (warp == 9) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -251,9 +281,13 @@ void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
   *NT = (per + 15) / 16 * 16;
 }
 
-size_t smem_bytes(int NH, int NT) {
-  return (size_t)kStages * (kABytes + NT * 128) + (size_t)NH * NT * 12 + (2 * kStages + 1) * 8 + 16;
+size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + (2 * kMaxStages + 2) * 8 + 16; }
+int stages_for(int NH, int NT) {
+  const size_t budget = 227 * 1024 - 1024;  // dynamic shared memory per CTA, less the alignment slack
+  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(2 * kABytes + NT * 128));
+  return std::min(st, kMaxStages);
 }
+size_t smem_bytes(int NH, int NT) { return (size_t)stages_for(NH, NT) * (2 * kABytes + NT * 128) + smem_fixed(NH, NT); }
 
 TcPlan* get_plan(pawfe_ctx* c) {
   if (c->tc_plan) return (TcPlan*)c->tc_plan;
@@ -312,9 +346,11 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.kchunks = (c->ldk + kChunkK - 1) / kChunkK;
   a.ksteps_last = (c->ldk - (a.kchunks - 1) * kChunkK) / 8;
   a.nvt = (B + kTileV - 1) / kTileV;
-  a.ntiles = c->ncell * a.nvt * a.NH;
+  a.nvg = (a.nvt + 1) / 2;
+  a.ntiles = c->ncell * a.nvg * a.NH;
+  a.stages = stages_for(p->NH, p->NT);
   uint32_t cols = 32;
-  while ((int)cols < a.NT) cols <<= 1;
+  while ((int)cols < std::min(a.nvt, 2) * a.NT) cols <<= 1;
   a.tmem_cols = cols;
   a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
   a.scale_mode = 0;
@@ -338,12 +374,7 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
       a.ext_ksteps = ext->ksteps;
     }
   }
-  a.dbg = 0;
-#ifdef PAWFE_TC_DEBUG
-  a.dbg = getenv("PAWFE_TC_DBG") ? atoi(getenv("PAWFE_TC_DBG")) : 0;
-  if (a.dbg & 1) a.idesc = ptx::idesc_tf32(kTileV, a.NT, 0, 0);
-#endif
-  int grid = std::min(a.ntiles, 2 * c->sm_count);
+  int grid = std::min(a.ntiles, c->sm_count);
   k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT), c->stream>>>(p->tmapH, a.ext_start ? p->tmapE : p->tmapH, a);
   KERNEL_CHECK(c, "k_cell_tcgen05");
   return PAWFE_OK;
