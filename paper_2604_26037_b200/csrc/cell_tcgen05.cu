@@ -45,15 +45,34 @@ struct TcArgs {
   int scale_mode;            // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
   // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
   const int* ext_start; const int* ext_atom; const float* Wcat; long ldw; int ext_ksteps;
+  int dbg;  // timing experiments only (PAWFE_TC_DBG): 1 plain stores, 2 no output, 4 no gather loads
 };
 
 struct TcPlan {
   CUtensorMap tmapH;
   CUtensorMap tmapE;             // K-extension blocks [chunk * n + I][32], built on first use for ext_ptr
   const void* ext_ptr = nullptr;
+  float* d_H32t = nullptr;       // cell matrices re-tiled for streaming: [cell][half][K chunk][NT rows][32] floats
   int NT = 0, NH = 0;
   bool ok = false;
 };
+
+// Re-tile the row-major FP32 cell matrices so that every (cell, half, K chunk) block the kernel loads is one
+// contiguous NT x 128-byte region of HBM (row-major [cell][n][ldk] gives NT scattered 128-byte pieces per load,
+// which costs DRAM page locality).  Rows >= n and columns >= n are zero.
+__global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH, int NT, int kchunks, long total,
+                             float* __restrict__ out) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+    const int kk = (int)(i & 31);
+    long t = i >> 5;
+    const int r = (int)(t % NT); t /= NT;
+    const int ch = (int)(t % kchunks); t /= kchunks;
+    const int half = (int)(t % NH);
+    const long cell = t / NH;
+    const int I = half * NT + r, k = ch * 32 + kk;
+    out[i] = (I < n && k < n) ? H[(cell * n + I) * ldk + k] : 0.f;
+  }
+}
 
 __device__ __forceinline__ void bar_sync_128(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
@@ -69,7 +88,8 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
   long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows (-1: none)
   long* eJ = gJ + a.NH * a.NT;                                            // [NT] output rows of this half
   float* eS = reinterpret_cast<float*>(eJ + a.NT);                        // [NT] output scale
-  uint64_t* full = reinterpret_cast<uint64_t*>(eS + a.NT);                // [stages]
+  float* stage_epi = eS + a.NT;                                           // [4 warps][32 nodes][32 vectors]
+  uint64_t* full = reinterpret_cast<uint64_t*>(stage_epi + 4 * 32 * 32);  // [stages]
   uint64_t* empty = full + kMaxStages;                                    // [stages]
   uint64_t* accum_full = empty + kMaxStages;
   uint64_t* accum_empty = accum_full + 1;
@@ -124,27 +144,50 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
       ptx::mbar_wait(accum_full, tile_iter & 1);
       ptx::tc_fence_after_sync();
       const int ncols = min(a.NT, a.n - half * a.NT);
+      // Each warp owns 32 vectors (TMEM lanes).  32 output nodes at a time: TMEM -> registers (lane = vector) ->
+      // scaled -> staging tile [node][vector] in shared memory -> each thread takes 4 consecutive vectors of one
+      // node and issues ONE 16-byte vector reduction (REDG.128): 4x fewer atomic lane-operations than scalar adds.
+      float* stg = stage_epi + warp * (32 * 32);
+      const int sub = lane >> 3, v4 = (lane & 7) * 4;
       for (int j = 0; j < nv; ++j) {
-        const int v = v0 + j * kTileV + warp * 32 + lane;
-        const bool vok = v < a.B;
-        char* yv = reinterpret_cast<char*>(a.Y + v);
+        if (a.dbg & 16) break;
+        const int vb = v0 + j * kTileV + warp * 32;
+        if (vb >= a.B) break;                       // warp-uniform: this warp's vectors are beyond the block
+        const bool vok = vb + v4 < a.B;             // B % 4 == 0: a float4 is all in or all out
+        char* yv = reinterpret_cast<char*>(a.Y + vb + v4);
         for (int col0 = 0; col0 < ncols; col0 += 32) {
           uint32_t r[32];
           const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(j * a.NT + col0);
           ptx::tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(&r[0]));
           if (col0 + 16 < ncols) ptx::tmem_ld16(taddr + 16, *reinterpret_cast<uint32_t(*)[16]>(&r[16]));
           ptx::tmem_ld_wait();
+          const int nq = min(32, ncols - col0);
+#pragma unroll
+          for (int q = 0; q < 32; q += 4) {
+            if (q < nq) {
+              const float4 sc = *reinterpret_cast<const float4*>(&eS[col0 + q]);
+              stg[(q + 0) * 32 + lane] = sc.x * __uint_as_float(r[q + 0]);
+              stg[(q + 1) * 32 + lane] = sc.y * __uint_as_float(r[q + 1]);
+              stg[(q + 2) * 32 + lane] = sc.z * __uint_as_float(r[q + 2]);
+              stg[(q + 3) * 32 + lane] = sc.w * __uint_as_float(r[q + 3]);
+            }
+          }
+          __syncwarp();
           if (vok) {
 #pragma unroll
-            for (int q = 0; q < 32; q += 2) {
-              if (col0 + q < ncols) {   // ncols is even or the odd tail column has offset -1
-                const longlong2 off = *reinterpret_cast<const longlong2*>(&eJ[col0 + q]);
-                const float2 sc = *reinterpret_cast<const float2*>(&eS[col0 + q]);
-                if (off.x >= 0) atomicAdd(reinterpret_cast<float*>(yv + off.x), sc.x * __uint_as_float(r[q]));
-                if (off.y >= 0) atomicAdd(reinterpret_cast<float*>(yv + off.y), sc.y * __uint_as_float(r[q + 1]));
+            for (int i = 0; i < 8; ++i) {
+              const int q = sub + 4 * i;
+              if (q < nq) {
+                const long off = eJ[col0 + q];
+                if (off >= 0) {
+                  const float4 val = *reinterpret_cast<const float4*>(&stg[q * 32 + v4]);
+                  if (a.dbg & 1) *reinterpret_cast<float4*>(yv + off) = val;
+                  else if (!(a.dbg & 2)) ptx::red_add_v4(reinterpret_cast<float*>(yv + off), val);
+                }
               }
             }
           }
+          __syncwarp();
         }
       }
       ptx::tc_fence_before_sync();
@@ -183,7 +226,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
             for (int i = 0; i < 8; ++i) {
               const long off = (c * kChunkK + wg + 4 * i < a.NH * a.NT) ? offs[4 * i] : -1;
               const bool ok = vok && off >= 0;
-              ptx::cp_async16(abase + j * kABytes + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
+              if (!(a.dbg & 4)) ptx::cp_async16(abase + j * kABytes + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
             }
           }
         } else {
@@ -196,21 +239,10 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
               ptx::cp_async16(abase + j * kABytes + i * 512, ok ? wrows + (long)(4 * i) * a.ldw + v : a.X, ok ? 16u : 0u);
           }
         }
-        ptx::cp_async_commit();
-        if (c >= 2) {
-          ptx::cp_async_wait<2>();
-          ptx::fence_proxy_async_smem();
-          ptx::mbar_arrive(&full[(it + c - 2) % a.stages]);
-        }
+        // arrival on full[s] fires when all of this thread's copies above have landed: no wait here, the thread
+        // goes straight on to the next chunk (gated only by that stage being free)
+        ptx::cp_async_mbar_arrive_noinc(&full[s]);
       }
-      if (nchunks >= 2) {
-        ptx::cp_async_wait<1>();
-        ptx::fence_proxy_async_smem();
-        ptx::mbar_arrive(&full[(it + nchunks - 2) % a.stages]);
-      }
-      ptx::cp_async_wait<0>();
-      ptx::fence_proxy_async_smem();
-      ptx::mbar_arrive(&full[(it + nchunks - 1) % a.stages]);
     } else if (warp == 8) {
       // ================= TMA producer: H^e row block (or K-extension block), one K chunk per stage =================
       if (lane == 0) {
@@ -220,7 +252,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
           ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
           const uint32_t dst = ptx::smem_u32(smem + s * sbytes + abytes);
           if (c < a.kchunks)
-            ptx::tma_load_2d(dst, &tmapH, c * kChunkK, cell * a.n + half * a.NT, &full[s]);
+            ptx::tma_load_2d(dst, &tmapH, 0, ((cell * a.NH + half) * a.kchunks + c) * a.NT, &full[s]);
           else
             ptx::tma_load_2d(dst, &tmapE, 0, (ext0 + c - a.kchunks) * a.n + half * a.NT, &full[s]);
         }
@@ -234,6 +266,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
         for (int c = 0; c < nchunks; ++c) {
           const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
           ptx::mbar_wait(&full[s], ph);
+          ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes of the A tiles -> tensor-core (async proxy) reads
           ptx::tc_fence_after_sync();
           const uint32_t abase = ptx::smem_u32(smem + s * sbytes), bbase = abase + abytes;
           const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
@@ -244,7 +277,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
               // A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
               // 512 B apart (SBO); one K step = 8 rows = 1024 B
               const uint64_t adesc = ptx::smem_desc(abase + j * kABytes + ks * 1024, 4096, 512, 1);
-              ptx::mma_tf32_ss(tmem_base + (uint32_t)(j * a.NT), adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+              if (!(a.dbg & 8)) ptx::mma_tf32_ss(tmem_base + (uint32_t)(j * a.NT), adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
             }
           }
           ptx::mma_commit(&empty[s]);
@@ -281,7 +314,7 @@ void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
   *NT = (per + 15) / 16 * 16;
 }
 
-size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + (2 * kMaxStages + 2) * 8 + 16; }
+size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 2) * 8 + 16; }
 int stages_for(int NH, int NT) {
   const size_t budget = 227 * 1024 - 1024;  // dynamic shared memory per CTA, less the alignment slack
   int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(2 * kABytes + NT * 128));
@@ -296,11 +329,17 @@ TcPlan* get_plan(pawfe_ctx* c) {
   shape_for(c, &p->NH, &p->NT);
   EncodeTiledFn enc = get_encode();
   if (!enc || !c->d_H32) return p;
-  cuuint64_t dims[2] = {(cuuint64_t)c->ldk, (cuuint64_t)c->ncell * c->n};
-  cuuint64_t strides[1] = {(cuuint64_t)c->ldk * sizeof(float)};
+  const int kchunks = (c->ldk + kChunkK - 1) / kChunkK;
+  const long rows = (long)c->ncell * p->NH * kchunks * p->NT;
+  if (cudaMalloc((void**)&p->d_H32t, (size_t)rows * 32 * sizeof(float)) != cudaSuccess) { cudaGetLastError(); p->d_H32t = nullptr; return p; }
+  k_retile_h32<<<8 * c->sm_count, 256, 0, c->stream>>>((const float*)c->d_H32, c->n, c->ldk, p->NH, p->NT, kchunks, rows * 32, p->d_H32t);
+  c->launches++;
+  if (cudaGetLastError() != cudaSuccess) return p;
+  cuuint64_t dims[2] = {32, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {32 * sizeof(float)};
   cuuint32_t box[2] = {(cuuint32_t)kChunkK, (cuuint32_t)p->NT};
   cuuint32_t estr[2] = {1, 1};
-  CUresult r = enc(&p->tmapH, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c->d_H32, dims, strides, box, estr,
+  CUresult r = enc(&p->tmapH, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d_H32t, dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return p;
@@ -321,7 +360,7 @@ TcPlan* get_plan(pawfe_ctx* c) {
 }  // namespace
 
 void tc_invalidate(pawfe_ctx* c) {
-  if (c->tc_plan) { delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
+  if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
 }
 
 bool tc_supported(const pawfe_ctx* c, int B) {
@@ -374,6 +413,7 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
       a.ext_ksteps = ext->ksteps;
     }
   }
+  { const char* d = getenv("PAWFE_TC_DBG"); a.dbg = d ? atoi(d) : 0; }
   int grid = std::min(a.ntiles, c->sm_count);
   k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT), c->stream>>>(p->tmapH, a.ext_start ? p->tmapE : p->tmapH, a);
   KERNEL_CHECK(c, "k_cell_tcgen05");

@@ -125,7 +125,7 @@ extern "C" pawfe_status pawfe_mesh_create(pawfe_ctx* c, const int ncells[3], con
   pawfe_free_atoms(c); pawfe_free_pot(c); pawfe_free_mesh(c);
   c->p = p; c->n1 = p + 1; c->n = c->n1 * c->n1 * c->n1; c->bc = (int)bc;
   c->cplx = (kpt != nullptr);
-  c->ldk = (c->n + 7) / 8 * 8;
+  c->ldk = (c->n + 31) / 32 * 32;  // 128-byte rows: every TMA box row of the FP32 cell matrices is one aligned line
   long M = 1; int ncell = 1;
   for (int d = 0; d < 3; ++d) {
     c->nc[d] = ncells[d]; c->box[d] = box[d]; c->h[d] = box[d] / ncells[d];
