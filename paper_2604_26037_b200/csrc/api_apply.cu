@@ -160,6 +160,13 @@ pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, l
   return pawfe_apply_nonlocal<TX, TY, TC>(c, OpData<TC>::dSinv(c), -1.0, X, ldx, 1, Y, ldy, 1, B);
 }
 
+template <typename RX>
+pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double* Y, long ldy, int B) {
+  return launch_dmma<RX, false>(c, (const double*)c->d_H64, (long)c->n * c->n, X, ldx, Y, ldy, B, 1.0);
+}
+template pawfe_status pawfe_cell_product_fp64<float>(pawfe_ctx*, const float*, long, double*, long, int);
+template pawfe_status pawfe_cell_product_fp64<double>(pawfe_ctx*, const double*, long, double*, long, int);
+
 // explicit instantiations used by the other translation units
 #define INST(TX, TY, TC)                                                                                          \
   template pawfe_status pawfe_apply_HS<TX, TY, TC>(pawfe_ctx*, int, bool, const TX*, long, TY*, long, int);       \

@@ -51,7 +51,8 @@ pawfe_status ensure_scalars(pawfe_ctx* c, size_t doubles) {
 
 // Step 1 and the Lambda recurrences of Alg. 2 on the host in FP64 (L257, L264, L275).  Fills a pinned staging slot,
 // starts its copy to the device and returns the per-step coefficients:
-//   device scalars ds: [0, B) Lambda;  [(th-1) B, th B) a_th Lambda_Y (th = 2..m);  [m B, (m+1) B) final Lambda_Y
+//   device scalars ds: [0, B) Lambda;  [(th-1) B, th B) a_th Lambda_Y (th = 2..m);  [m B, (m+1) B) final Lambda_Y;
+//   [(m+1) B, (m+2) B) -Lambda
 struct FilterScalars {
   const double* ds = nullptr;
   std::vector<double> as, acs, zzs;
@@ -63,7 +64,7 @@ pawfe_status filter_scalars(pawfe_ctx* c, int m, double b0, double bW, double bU
   const double e = 0.5 * (bU - bW), cc = 0.5 * (bU + bW);
   double zeta = e / (b0 - cc);
   const double gamma = 2.0 / zeta;
-  TRY(ensure_scalars(c, (size_t)(m + 1) * B));
+  TRY(ensure_scalars(c, (size_t)(m + 2) * B));
   const int slot = c->scal_next;
   c->scal_next = (slot + 1) % pawfe_ctx::kScalSlots;
   CUDA_TRY(c, cudaEventSynchronize(c->scal_ev[slot]));  // the slot's previous copy has been consumed
@@ -85,8 +86,8 @@ pawfe_status filter_scalars(pawfe_ctx* c, int m, double b0, double bW, double bU
     }
     zeta = zeta1;
   }
-  for (int v = 0; v < B; ++v) hs[(size_t)m * B + v] = LY[v];
-  CUDA_TRY(c, cudaMemcpyAsync(ds, hs, (size_t)(m + 1) * B * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  for (int v = 0; v < B; ++v) { hs[(size_t)m * B + v] = LY[v]; hs[(size_t)(m + 1) * B + v] = -lambda[v]; }
+  CUDA_TRY(c, cudaMemcpyAsync(ds, hs, (size_t)(m + 2) * B * sizeof(double), cudaMemcpyHostToDevice, c->stream));
   CUDA_TRY(c, cudaEventRecord(c->scal_ev[slot], c->stream));
   out->ds = ds; out->z_over_e = z_over_e;
   return PAWFE_OK;

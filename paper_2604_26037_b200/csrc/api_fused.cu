@@ -6,6 +6,7 @@
 #include "host_util.h"
 #include "api_internal.h"
 #include "apply_impl.h"
+#include "setup_fp64.cuh"
 #include <algorithm>
 #include <cmath>
 #include <set>
@@ -24,6 +25,8 @@ struct FusedPlan {
   int Bcap = 0; long ldw = 0;
   float* d_P1 = nullptr;        // [natoms][npj][ldw]
   float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
+  double* d_P64 = nullptr;      // [natoms][npj][ldw] FP64 projections of the residual set-up
+  double* d_W64 = nullptr;      // [natoms][npj][ldw] (D - Lambda dS) P
 };
 
 namespace {
@@ -54,7 +57,7 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
             const int* __restrict__ aps, const int* __restrict__ pair_cell, const double* __restrict__ Cd64,
             int npj, const double* __restrict__ H64, const int* __restrict__ cell_pair_start,
             const int* __restrict__ cell_pair_idx, const int* __restrict__ pair_atom,
-            const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
+            const int* __restrict__ nb_start, const int* __restrict__ nb_atom, int NH, int NT,
             float* __restrict__ Bext, double* __restrict__ G) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* Zs = reinterpret_cast<double*>(smem_raw);  // [n][npj]
@@ -100,7 +103,12 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const int prb = find_pair(aps, pair_cell, b, e);
   const double* He = H64 + (long)e * n * n;
-  float* Bx = Bext + (long)x * n * 32;
+  // block layout of the cell kernel's operand stream: [x][half][NT rows][32], 128-byte swizzled per row
+  // (16-byte piece j of row r stored at j ^ (r % 8)); rows I >= n stay zero
+  auto bidx = [&](int I, int k) -> long {
+    const int half = I / NT, r = I - half * NT;
+    return (((long)x * NH + half) * NT + r) * 32 + ((((k >> 2) ^ (r & 7)) << 2) | (k & 3));
+  };
   for (int I = w; I < n; I += nw) {
     double acc[PAWFE_MAX_NPJ];
 #pragma unroll
@@ -116,12 +124,12 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
       if (be < npj) {
         double s = acc[be];
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) Bx[I * 32 + be] = (float)(-s);
+        if (lane == 0) Bext[bidx(I, be)] = (float)(-s);
       }
     for (int k = npj + lane; k < 32; k += 32) {
       float v = 0.f;
       if (k < 2 * npj && prb >= 0) v = (float)Cd64[((long)prb * npj + (k - npj)) * n + I];
-      Bx[I * 32 + k] = v;
+      Bext[bidx(I, k)] = v;
     }
   }
   // ---- phase 3: G^{ab} contributions of this cell ----
@@ -145,57 +153,68 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
 //   grid = (npairs, ceil(B/128)), block = 256 (8 warps over rows, lane = 4 consecutive vectors).
 //   dynamic smem: n longs + npj*n floats + 16*128 floats.  P must be zero on entry.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+template <int NPJ>
+__global__ void __launch_bounds__(256, (NPJ <= 9 ? 3 : 2))
 k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
-        const float* __restrict__ Cd, int npj, const float* __restrict__ X, long ldx, int B,
+        const float* __restrict__ Cd, const float* __restrict__ X, long ldx, int B,
         float* __restrict__ P, long ldp) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = md.n, n1 = md.n1;
-  long* nodeJ = reinterpret_cast<long*>(smem_raw);
-  float* Cs = reinterpret_cast<float*>(nodeJ + n);     // [npj][n]
-  float* red = Cs + (size_t)npj * n;                   // [16][128]
+  long* nodeO = reinterpret_cast<long*>(smem_raw);     // byte offset of the node's row, -1: masked
+  float* Cs = reinterpret_cast<float*>(nodeO + (n + 1) / 2 * 2);     // [NPJ][n], 16-byte aligned
+  float* red = Cs + ((size_t)NPJ * n + 3) / 4 * 4;     // [NPJ][128], 16-byte aligned
   const int pr = blockIdx.x, a = pair_atom[pr];
   int cx, cy, cz;
   mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
   for (int I = threadIdx.x; I < n; I += blockDim.x) {
     int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
     long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-    if (md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0) J = -1;
-    nodeJ[I] = J;
+    nodeO[I] = (md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0) ? -1 : J * ldx * 4;
   }
-  for (int i = threadIdx.x; i < npj * n; i += blockDim.x) Cs[i] = Cd[(long)pr * npj * n + i];
-  for (int i = threadIdx.x; i < 16 * 128; i += blockDim.x) red[i] = 0.f;
+  for (int i = threadIdx.x; i < NPJ * n; i += blockDim.x) Cs[i] = Cd[(long)pr * NPJ * n + i];
+  for (int i = threadIdx.x; i < NPJ * 128; i += blockDim.x) red[i] = 0.f;
   __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int v = blockIdx.y * 128 + lane * 4;
-  float4 acc[PAWFE_MAX_NPJ];
+  float4 acc[NPJ];
 #pragma unroll
-  for (int al = 0; al < PAWFE_MAX_NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int al = 0; al < NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
   if (v < B) {
-#pragma unroll 4
-    for (int I = w; I < n; I += 8) {
-      const long J = nodeJ[I];
-      if (J < 0) continue;
-      const float4 x = __ldg(reinterpret_cast<const float4*>(X + J * ldx + v));
+    const char* xv = reinterpret_cast<const char*>(X + v);
+    // rows w, w + 8, ... ; four independent 16-byte loads in flight per thread before the first use
+    for (int I0 = w; I0 < n; I0 += 32) {
+      float4 x[4];
 #pragma unroll
-      for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
-        if (al < npj) {
+      for (int u = 0; u < 4; ++u) {
+        const int I = I0 + 8 * u;
+        const long off = I < n ? nodeO[I] : -1;
+        x[u] = off >= 0 ? __ldg(reinterpret_cast<const float4*>(xv + off)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int I = min(I0 + 8 * u, n - 1);   // x[u] is zero beyond n
+#pragma unroll
+        for (int al = 0; al < NPJ; ++al) {
           const float cv = Cs[al * n + I];
-          acc[al].x = fmaf(cv, x.x, acc[al].x); acc[al].y = fmaf(cv, x.y, acc[al].y);
-          acc[al].z = fmaf(cv, x.z, acc[al].z); acc[al].w = fmaf(cv, x.w, acc[al].w);
+          acc[al].x = fmaf(cv, x[u].x, acc[al].x); acc[al].y = fmaf(cv, x[u].y, acc[al].y);
+          acc[al].z = fmaf(cv, x[u].z, acc[al].z); acc[al].w = fmaf(cv, x[u].w, acc[al].w);
         }
+      }
     }
 #pragma unroll
-    for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
-      if (al < npj) {
-        float* r = red + al * 128 + lane * 4;
-        atomicAdd(r + 0, acc[al].x); atomicAdd(r + 1, acc[al].y); atomicAdd(r + 2, acc[al].z); atomicAdd(r + 3, acc[al].w);
-      }
+    for (int al = 0; al < NPJ; ++al) {
+      float* r = red + al * 128 + lane * 4;
+      atomicAdd(r + 0, acc[al].x); atomicAdd(r + 1, acc[al].y); atomicAdd(r + 2, acc[al].z); atomicAdd(r + 3, acc[al].w);
+    }
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < npj * 128; i += blockDim.x) {
-    const int al = i >> 7, vv = blockIdx.y * 128 + (i & 127);
-    if (vv < B) atomicAdd(P + ((long)a * npj + al) * ldp + vv, red[i]);
+  for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
+    const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
+    if (vv < B) {
+      const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
+      float* dst = P + ((long)a * NPJ + al) * ldp + vv;
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
+    }
   }
 }
 
@@ -369,7 +388,7 @@ void free_plan(FusedPlan* p) {
   if (!p) return;
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
   cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD);
-  cudaFree(p->d_P1); cudaFree(p->d_Wcat);
+  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
   delete p;
 }
 
@@ -433,7 +452,10 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   TRYP(upload(c, &p->d_ext_start, es)); TRYP(upload(c, &p->d_ext_atom, ea)); TRYP(upload(c, &d_ec, ec));
   TRYP(upload(c, &d_cps, cps)); TRYP(upload(c, &d_cpi, cpi));
   TRYP(upload(c, &p->d_nb_start, ns)); TRYP(upload(c, &p->d_nb_atom, na));
-  TRYP(dev_alloc(c, &p->d_Bext, (size_t)p->nchunks * n * 32));
+  int NH = 1, NT = n;
+  tc_shape(c, &NH, &NT);
+  TRYP(dev_alloc(c, &p->d_Bext, (size_t)p->nchunks * NH * NT * 32));
+  cudaMemsetAsync(p->d_Bext, 0, (size_t)p->nchunks * NH * NT * 32 * sizeof(float), c->stream);
   TRYP(dev_alloc(c, &d_G, (size_t)nnb * npj * npj));
   cudaMemsetAsync(d_G, 0, (size_t)nnb * npj * npj * sizeof(double), c->stream);
   size_t smem = (size_t)n * npj * sizeof(double);
@@ -441,7 +463,7 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   if (e == cudaSuccess) {
     k_build_ext<<<(unsigned)p->nchunks, 256, smem, c->stream>>>(
         c->md, d_ec, p->d_ext_atom, c->d_atom_pair_start, c->d_pair_cell, (const double*)c->d_Cd64, npj,
-        (const double*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, p->d_Bext, d_G);
+        (const double*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, NH, NT, p->d_Bext, d_G);
     c->launches++;
     e = cudaGetLastError();
   }
@@ -479,11 +501,14 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
 pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int B) {
   if (B <= p->Bcap) return PAWFE_OK;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  cudaFree(p->d_P1); cudaFree(p->d_Wcat); p->d_P1 = p->d_Wcat = nullptr; p->Bcap = 0;
+  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
+  p->d_P1 = p->d_Wcat = nullptr; p->d_P64 = p->d_W64 = nullptr; p->Bcap = 0;
   const long ldw = roundup4(B);
   const size_t na = (size_t)std::max(1, c->natoms);
   TRY(dev_alloc(c, &p->d_P1, na * c->npj * ldw));
   TRY(dev_alloc(c, &p->d_Wcat, na * 32 * ldw));
+  TRY(dev_alloc(c, &p->d_P64, na * c->npj * ldw));
+  TRY(dev_alloc(c, &p->d_W64, na * c->npj * ldw));
   CUDA_TRY(c, cudaMemsetAsync(p->d_Wcat, 0, na * 32 * ldw * sizeof(float), c->stream));
   p->Bcap = B; p->ldw = ldw;
   return PAWFE_OK;
@@ -494,17 +519,65 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
   CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
-  size_t smem = (size_t)n * 8 + (size_t)npj * n * 4 + 16 * 128 * 4;
-  static size_t smem_attr = 0;
-  if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
-  k_proj2<<<dim3((unsigned)c->npairs, ceil_div(B, 128)), 256, smem, c->stream>>>(
-      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, npj, X, ldx, B, p->d_P1, p->ldw);
+  size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4;
+  dim3 grid((unsigned)c->npairs, ceil_div(B, 128));
+#define LAUNCH_PROJ2(NPJ)                                                                                            \
+  do {                                                                                                               \
+    static size_t smem_attr = 0;                                                                                     \
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj2<NPJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; } \
+    k_proj2<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw); \
+  } while (0)
+  switch (npj) {
+    case 1: LAUNCH_PROJ2(1); break;   case 2: LAUNCH_PROJ2(2); break;   case 3: LAUNCH_PROJ2(3); break;
+    case 4: LAUNCH_PROJ2(4); break;   case 5: LAUNCH_PROJ2(5); break;   case 6: LAUNCH_PROJ2(6); break;
+    case 7: LAUNCH_PROJ2(7); break;   case 8: LAUNCH_PROJ2(8); break;   case 9: LAUNCH_PROJ2(9); break;
+    case 10: LAUNCH_PROJ2(10); break; case 11: LAUNCH_PROJ2(11); break; case 12: LAUNCH_PROJ2(12); break;
+    case 13: LAUNCH_PROJ2(13); break; case 14: LAUNCH_PROJ2(14); break; case 15: LAUNCH_PROJ2(15); break;
+    default: LAUNCH_PROJ2(16); break;
+  }
+#undef LAUNCH_PROJ2
   KERNEL_CHECK(c, "k_proj2");
   k_couple<<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
       npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
       p->d_GD, p->d_Wcat, p->ldw);
   KERNEL_CHECK(c, "k_couple");
   return PAWFE_OK;
+}
+
+// Y += C (D P - dS P Lambda), P = C^T X, all FP64 (non-local parts of H X - S X Lambda with one projection)
+template <int NPJ>
+pawfe_status setup_nonlocal64_t(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, const double* lam,
+                                double* Y, long ldy) {
+  const int n = c->n;
+  CUDA_TRY(c, cudaMemsetAsync(p->d_P64, 0, (size_t)c->natoms * NPJ * p->ldw * sizeof(double), c->stream));
+  dim3 grid((unsigned)c->npairs, ceil_div(B, 64));
+  {
+    const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8 + (size_t)NPJ * 64 * 8;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj64<NPJ, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_proj64<NPJ, float><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const double*)c->d_Cd64, X, ldx, B, p->d_P64, p->ldw);
+    KERNEL_CHECK(c, "k_proj64");
+  }
+  k_couple64<<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(NPJ, p->d_P64, p->ldw, B, (const double*)c->d_D64,
+                                                                       (const double*)c->d_dS64, lam, p->d_W64);
+  KERNEL_CHECK(c, "k_couple64");
+  {
+    const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatter64<NPJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_scatter64<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const double*)c->d_Cd64, p->d_W64, p->ldw, B, Y, ldy);
+    KERNEL_CHECK(c, "k_scatter64");
+  }
+  return PAWFE_OK;
+}
+pawfe_status setup_nonlocal64(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, const double* lam, double* Y, long ldy) {
+  switch (c->npj) {
+#define CASE_NL(N) case N: return setup_nonlocal64_t<N>(c, p, X, ldx, B, lam, Y, ldy);
+    CASE_NL(1) CASE_NL(2) CASE_NL(3) CASE_NL(4) CASE_NL(5) CASE_NL(6) CASE_NL(7) CASE_NL(8)
+    CASE_NL(9) CASE_NL(10) CASE_NL(11) CASE_NL(12) CASE_NL(13) CASE_NL(14) CASE_NL(15) CASE_NL(16)
+#undef CASE_NL
+  }
+  return PAWFE_EINVAL;
 }
 
 TcExt make_ext(const FusedPlan* p, int scale_mode) {
@@ -560,12 +633,22 @@ pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const doub
   double* SX = (double*)(ws + blk_d);
   float* RX = (float*)(ws + 2 * blk_d);
   float* RY = (float*)(ws + 2 * blk_d + blk_s);
-  // ---- step 2 (FP64): H X and S X ----
-  TRY((pawfe_apply_HS<float, double, double>(c, 0, false, X, ld, Yt, ldw, B)));
-  TRY((pawfe_apply_HS<float, double, double>(c, 1, false, X, ld, SX, ldw, B)));
+  // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda, fused (setup_fp64.cuh): S X is never stored ----
+  (void)SX;
+  CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
+  TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
+  {
+    const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_mass_sf<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
+        c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
+    KERNEL_CHECK(c, "k_mass_sf");
+  }
   const int gs = 8 * c->sm_count;
-  k_residual_init2<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, SX, ds, z_over_e, RX, RY);
-  KERNEL_CHECK(c, "k_residual_init2");
+  if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
+  k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, z_over_e, RX, RY);
+  KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
   TcExt x = make_ext(p, 1);
   const long nquads = c->M * (ldw / 4);

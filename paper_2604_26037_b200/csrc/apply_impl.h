@@ -12,3 +12,7 @@ pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, l
 // H apply in the storage type selected by prec (float / double, complex if the context is); picks the
 // tcgen05 kernel for the TF32 mode when it supports the shape.
 pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, long ldx, void* Y, long ldy, int B);
+
+// Y += sum_e P_e^T H^e (P_e X) in FP64 on the DMMA pipe, real contexts (no zeroing of Y, no non-local term).
+template <typename RX>
+pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double* Y, long ldy, int B);

@@ -73,6 +73,9 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int rg = warp & 3, vh = warp >> 2;
   const int nchunks = (n + KC - 1) / KC;
+  // n-tiles (8 real columns) of this warp that hold any column of the block: the others are skipped (ragged last tile)
+  int ntv = 0;
+  for (int nt = 0; nt < 4; ++nt) if (v0 + vh * 32 + nt * 8 < Wr) ntv = nt + 1;
 
   for (int r0 = 0; r0 < n; r0 += RB) {
     double acc[MT][4][2];
@@ -141,7 +144,7 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
       const double* As = reinterpret_cast<const double*>(st);
       const RX* Bs = reinterpret_cast<const RX*>(st + aBytes);
 #pragma unroll
-      for (int ks = 0; ks < KC / 4; ++ks) {
+      for (int ks = 0; ks < KC / 4 && ntv > 0; ++ks) {
         const int kk = ks * 4 + (lane & 3);
         double b[4], bi[4];
 #pragma unroll
@@ -161,14 +164,16 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
           if (CPLX) {
             const double2 a2 = *reinterpret_cast<const double2*>(As + row * strideA + kk * 2);
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt) {
-              dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.x, b[nt]);
-              dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.y, bi[nt]);
-            }
+            for (int nt = 0; nt < 4; ++nt)
+              if (nt < ntv) {
+                dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.x, b[nt]);
+                dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.y, bi[nt]);
+              }
           } else {
             const double a1 = As[row * strideA + kk];
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a1, b[nt]);
+            for (int nt = 0; nt < 4; ++nt)
+              if (nt < ntv) dmma884(acc[mt][nt][0], acc[mt][nt][1], a1, b[nt]);
           }
         }
       }

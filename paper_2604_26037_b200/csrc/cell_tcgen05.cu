@@ -37,14 +37,14 @@ struct TcArgs {
   float* Y; long ldy;
   int B; float alpha;
   int n, NH, NT, kchunks, ksteps_last;
-  int nvt;       // vector tiles of 128 in the block
-  int nvg;       // groups of up to 2 vector tiles (one CTA tile holds a group: both share every H^e load)
-  int ntiles;    // ncell * nvg * NH
+  int nvt;       // vector tiles of 128 in the block (processed one after the other inside a tile)
+  int ntiles;    // ncell * NH
   int stages;
-  uint32_t tmem_cols, idesc;
+  uint32_t tmem_cols, acc_stride, idesc;   // two accumulators of NT columns, acc_stride apart
   int scale_mode;            // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
   // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
   const int* ext_start; const int* ext_atom; const float* Wcat; long ldw; int ext_ksteps;
+  const float* H32t; const float* Bext;   // pre-swizzled, block-contiguous operand streams
   int dbg;  // timing experiments only (PAWFE_TC_DBG): 1 plain stores, 2 no output, 4 no gather loads
 };
 
@@ -70,36 +70,38 @@ __global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH
     const int half = (int)(t % NH);
     const long cell = t / NH;
     const int I = half * NT + r, k = ch * 32 + kk;
-    out[i] = (I < n && k < n) ? H[(cell * n + I) * ldk + k] : 0.f;
+    // 128-byte-swizzled image: 16-byte piece j of row r is stored at piece j ^ (r % 8), so that a plain contiguous
+    // bulk copy of the block lands in shared memory in the layout the K-major SW128 matrix descriptor expects
+    const long o = (i & ~31L) + ((((kk >> 2) ^ (r & 7)) << 2) | (kk & 3));
+    out[o] = (I < n && k < n) ? H[(cell * n + I) * ldk + k] : 0.f;
   }
 }
 
 __device__ __forceinline__ void bar_sync_128(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
-// Persistent CTAs (one per SM) loop over tiles (cell, vector group, node half).  Roles are decoupled across tiles:
-// the gather / TMA producers run ahead into the next tile through the shared-memory ring while the epilogue warps
-// drain the accumulators of the current one; the MMA issuer waits for the drained accumulator (accum_empty).
+// Persistent CTAs (one per SM) loop over tiles (cell, node half); inside a tile over the vector tiles of 128
+// ("subtiles").  The first vector tile of a tile streams its H^e half from HBM, the following ones re-read it
+// from L2.  Accumulators are double-buffered in tensor memory (subtile parity), so the assembly epilogue of one
+// subtile runs under the loads and MMAs of the next.  Roles are decoupled through mbarriers only.
 __global__ void __launch_bounds__(kThreads, 1)
 k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant__ CUtensorMap tmapE, const TcArgs a) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const int bbytes = a.NT * 128;
-  const int abytes = 2 * kABytes;                       // room for two vector tiles
-  const int sbytes = abytes + bbytes;                   // one stage: [A vt0][A vt1][B]
-  long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows (-1: none)
+  const int sbytes = kABytes + bbytes;                  // one stage: [A][B]
+  long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows: byte offset or -1
   long* eJ = gJ + a.NH * a.NT;                                            // [NT] output rows of this half
   float* eS = reinterpret_cast<float*>(eJ + a.NT);                        // [NT] output scale
   float* stage_epi = eS + a.NT;                                           // [4 warps][32 nodes][32 vectors]
   uint64_t* full = reinterpret_cast<uint64_t*>(stage_epi + 4 * 32 * 32);  // [stages]
   uint64_t* empty = full + kMaxStages;                                    // [stages]
-  uint64_t* accum_full = empty + kMaxStages;
-  uint64_t* accum_empty = accum_full + 1;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_empty + 1);
+  uint64_t* accum_full = empty + kMaxStages;                              // [2]
+  uint64_t* accum_empty = accum_full + 2;                                 // [2]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_empty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < a.stages; ++s) { ptx::mbar_init(&full[s], 128 + 1); ptx::mbar_init(&empty[s], 1); }
-    ptx::mbar_init(accum_full, 1);
-    ptx::mbar_init(accum_empty, 128);
+    for (int b = 0; b < 2; ++b) { ptx::mbar_init(&accum_full[b], 1); ptx::mbar_init(&accum_empty[b], 128); }
     ptx::fence_barrier_init();
   }
   if (warp == 8 && lane == 0) { ptx::prefetch_tmap(&tmapH); if (a.ext_start) ptx::prefetch_tmap(&tmapE); }
@@ -109,23 +111,19 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
   ptx::tc_fence_after_sync();
   const uint32_t tmem_base = *tmem_slot;
   const int n1 = a.md.n1;
-  const int per_cell = a.nvg * a.NH;
 
   uint32_t it = 0;        // running chunk counter (same sequence in every role)
-  uint32_t tile_iter = 0;
-  for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++tile_iter) {
-    const int cell = tile / per_cell;
-    const int rem = tile - cell * per_cell;
-    const int vg = rem / a.NH, half = rem - vg * a.NH;
-    const int v0 = vg * 2 * kTileV;
-    const int nv = min(2, a.nvt - 2 * vg);            // vector tiles in this group
+  uint32_t sub_iter = 0;  // running subtile counter: accumulator buffer = sub_iter & 1
+  for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+    const int cell = tile / a.NH;
+    const int half = tile - cell * a.NH;
     const int ext0 = a.ext_start ? a.ext_start[cell] : 0;
     const int nchunks = a.kchunks + (a.ext_start ? a.ext_start[cell + 1] - ext0 : 0);
     int cx, cy, cz;
     mesh_cell_coords(a.md, cell, &cx, &cy, &cz);
 
     if (warp < 4) {
-      // ================= epilogue: TMEM -> scaled atomic adds into Y (assembly, Fig. 2 step iv) =================
+      // ================= epilogue: TMEM -> scaled vector reductions into Y (assembly, Fig. 2 step iv) =================
       bar_sync_128(2);   // previous tile's readers of eJ / eS are done
       for (int I = threadIdx.x; I < a.NT; I += 128) {
         const int Ig = half * a.NT + I;
@@ -141,57 +139,58 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
         eJ[I] = J; eS[I] = sc;
       }
       bar_sync_128(2);
-      ptx::mbar_wait(accum_full, tile_iter & 1);
-      ptx::tc_fence_after_sync();
       const int ncols = min(a.NT, a.n - half * a.NT);
       // Each warp owns 32 vectors (TMEM lanes).  32 output nodes at a time: TMEM -> registers (lane = vector) ->
       // scaled -> staging tile [node][vector] in shared memory -> each thread takes 4 consecutive vectors of one
       // node and issues ONE 16-byte vector reduction (REDG.128): 4x fewer atomic lane-operations than scalar adds.
       float* stg = stage_epi + warp * (32 * 32);
       const int sub = lane >> 3, v4 = (lane & 7) * 4;
-      for (int j = 0; j < nv; ++j) {
-        if (a.dbg & 16) break;
-        const int vb = v0 + j * kTileV + warp * 32;
-        if (vb >= a.B) break;                       // warp-uniform: this warp's vectors are beyond the block
+      for (int vt = 0; vt < a.nvt; ++vt) {
+        const uint32_t buf = (sub_iter + vt) & 1, use = (sub_iter + vt) >> 1;
+        ptx::mbar_wait(&accum_full[buf], use & 1);
+        ptx::tc_fence_after_sync();
+        const int vb = vt * kTileV + warp * 32;
         const bool vok = vb + v4 < a.B;             // B % 4 == 0: a float4 is all in or all out
         char* yv = reinterpret_cast<char*>(a.Y + vb + v4);
-        for (int col0 = 0; col0 < ncols; col0 += 32) {
-          uint32_t r[32];
-          const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(j * a.NT + col0);
-          ptx::tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(&r[0]));
-          if (col0 + 16 < ncols) ptx::tmem_ld16(taddr + 16, *reinterpret_cast<uint32_t(*)[16]>(&r[16]));
-          ptx::tmem_ld_wait();
-          const int nq = min(32, ncols - col0);
+        if (vb < a.B && !(a.dbg & 16)) {
+          for (int col0 = 0; col0 < ncols; col0 += 32) {
+            uint32_t r[32];
+            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
+            ptx::tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(&r[0]));
+            if (col0 + 16 < ncols) ptx::tmem_ld16(taddr + 16, *reinterpret_cast<uint32_t(*)[16]>(&r[16]));
+            ptx::tmem_ld_wait();
+            const int nq = min(32, ncols - col0);
 #pragma unroll
-          for (int q = 0; q < 32; q += 4) {
-            if (q < nq) {
-              const float4 sc = *reinterpret_cast<const float4*>(&eS[col0 + q]);
-              stg[(q + 0) * 32 + lane] = sc.x * __uint_as_float(r[q + 0]);
-              stg[(q + 1) * 32 + lane] = sc.y * __uint_as_float(r[q + 1]);
-              stg[(q + 2) * 32 + lane] = sc.z * __uint_as_float(r[q + 2]);
-              stg[(q + 3) * 32 + lane] = sc.w * __uint_as_float(r[q + 3]);
-            }
-          }
-          __syncwarp();
-          if (vok) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const int q = sub + 4 * i;
+            for (int q = 0; q < 32; q += 4) {
               if (q < nq) {
-                const long off = eJ[col0 + q];
-                if (off >= 0) {
-                  const float4 val = *reinterpret_cast<const float4*>(&stg[q * 32 + v4]);
-                  if (a.dbg & 1) *reinterpret_cast<float4*>(yv + off) = val;
-                  else if (!(a.dbg & 2)) ptx::red_add_v4(reinterpret_cast<float*>(yv + off), val);
+                const float4 sc = *reinterpret_cast<const float4*>(&eS[col0 + q]);
+                stg[(q + 0) * 32 + lane] = sc.x * __uint_as_float(r[q + 0]);
+                stg[(q + 1) * 32 + lane] = sc.y * __uint_as_float(r[q + 1]);
+                stg[(q + 2) * 32 + lane] = sc.z * __uint_as_float(r[q + 2]);
+                stg[(q + 3) * 32 + lane] = sc.w * __uint_as_float(r[q + 3]);
+              }
+            }
+            __syncwarp();
+            if (vok) {
+#pragma unroll
+              for (int i = 0; i < 8; ++i) {
+                const int q = sub + 4 * i;
+                if (q < nq) {
+                  const long off = eJ[col0 + q];
+                  if (off >= 0) {
+                    const float4 val = *reinterpret_cast<const float4*>(&stg[q * 32 + v4]);
+                    if (a.dbg & 1) *reinterpret_cast<float4*>(yv + off) = val;
+                    else if (!(a.dbg & 2)) ptx::red_add_v4(reinterpret_cast<float*>(yv + off), val);
+                  }
                 }
               }
             }
+            __syncwarp();
           }
-          __syncwarp();
         }
+        ptx::tc_fence_before_sync();
+        ptx::mbar_arrive(&accum_empty[buf]);
       }
-      ptx::tc_fence_before_sync();
-      ptx::mbar_arrive(accum_empty);
     } else if (warp < 8) {
       // ================= gather producers: X rows -> swizzled MN-major A tiles (Fig. 2 step i) =================
       const int t = threadIdx.x - 128;  // 0..127
@@ -206,87 +205,92 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
         gJ[I] = J;
       }
       bar_sync_128(1);
-      // per-thread constants: this thread always copies 16-byte column lane of rows wg, wg + 4, ... of a chunk
+      // per-thread constants: this thread always copies 16-byte column `lane` of rows wg, wg + 4, ... of a chunk
       const int wg = t >> 5;                               // row within each group of 4
       const int vl = lane * 4;                             // first vector of the 16-byte piece inside the tile
       // MN-major tf32 layout (128-byte swizzle, 32-byte atoms): 32-vector column block cb at cb * 4096; row r at
       // r * 128; its four 32-byte chunks q stored at q ^ (r % 4); r % 4 == wg for every row this thread copies
       const uint32_t dst_thread = (lane >> 3) * 4096 + wg * 128 + (((((lane & 7) >> 1) ^ wg) << 5) | ((lane & 1) << 4));
-      for (int c = 0; c < nchunks; ++c) {
-        const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
-        ptx::mbar_wait(&empty[s], ph ^ 1);
-        const uint32_t abase = ptx::smem_u32(smem + s * sbytes) + dst_thread;
-        if (c < a.kchunks) {
-          const long* offs = gJ + c * kChunkK + wg;
-          for (int j = 0; j < nv; ++j) {
-            const int v = v0 + j * kTileV + vl;
-            const bool vok = v < a.B;
-            const char* xv = reinterpret_cast<const char*>(a.X + v);
+      uint32_t itc = it;
+      for (int vt = 0; vt < a.nvt; ++vt) {
+        const int v = vt * kTileV + vl;
+        const bool vok = v < a.B;
+        const char* xv = reinterpret_cast<const char*>(a.X + v);
+        for (int c = 0; c < nchunks; ++c, ++itc) {
+          const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
+          ptx::mbar_wait(&empty[s], ph ^ 1);
+          const uint32_t abase = ptx::smem_u32(smem + s * sbytes) + dst_thread;
+          if (c < a.kchunks) {
+            const long* offs = gJ + c * kChunkK + wg;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               const long off = (c * kChunkK + wg + 4 * i < a.NH * a.NT) ? offs[4 * i] : -1;
               const bool ok = vok && off >= 0;
-              if (!(a.dbg & 4)) ptx::cp_async16(abase + j * kABytes + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
+              if (!(a.dbg & 4)) ptx::cp_async16(abase + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
             }
-          }
-        } else {
-          const float* wrows = a.Wcat + ((long)a.ext_atom[ext0 + c - a.kchunks] * 32 + wg) * a.ldw;
-          for (int j = 0; j < nv; ++j) {
-            const int v = v0 + j * kTileV + vl;
-            const bool ok = v < a.B;
+          } else {
+            const float* wrows = a.Wcat + ((long)a.ext_atom[ext0 + c - a.kchunks] * 32 + wg) * a.ldw + v;
 #pragma unroll
             for (int i = 0; i < 8; ++i)
-              ptx::cp_async16(abase + j * kABytes + i * 512, ok ? wrows + (long)(4 * i) * a.ldw + v : a.X, ok ? 16u : 0u);
+              ptx::cp_async16(abase + i * 512, vok ? wrows + (long)(4 * i) * a.ldw : a.X, vok ? 16u : 0u);
           }
+          // arrival on full[s] fires when all of this thread's copies above have landed: no wait here, the thread
+          // goes straight on to the next chunk (gated only by that stage being free)
+          ptx::cp_async_mbar_arrive_noinc(&full[s]);
         }
-        // arrival on full[s] fires when all of this thread's copies above have landed: no wait here, the thread
-        // goes straight on to the next chunk (gated only by that stage being free)
-        ptx::cp_async_mbar_arrive_noinc(&full[s]);
       }
     } else if (warp == 8) {
       // ================= TMA producer: H^e row block (or K-extension block), one K chunk per stage =================
       if (lane == 0) {
-        for (int c = 0; c < nchunks; ++c) {
-          const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
-          ptx::mbar_wait(&empty[s], ph ^ 1);
-          ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
-          const uint32_t dst = ptx::smem_u32(smem + s * sbytes + abytes);
-          if (c < a.kchunks)
-            ptx::tma_load_2d(dst, &tmapH, 0, ((cell * a.NH + half) * a.kchunks + c) * a.NT, &full[s]);
-          else
-            ptx::tma_load_2d(dst, &tmapE, 0, (ext0 + c - a.kchunks) * a.n + half * a.NT, &full[s]);
-        }
+        uint32_t itc = it;
+        for (int vt = 0; vt < a.nvt; ++vt)
+          for (int c = 0; c < nchunks; ++c, ++itc) {
+            const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
+            ptx::mbar_wait(&empty[s], ph ^ 1);
+            ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
+            const uint32_t dst = ptx::smem_u32(smem + s * sbytes + kABytes);
+            // both operand streams are stored pre-swizzled and block-contiguous: one linear bulk copy per chunk
+            const float* src = (c < a.kchunks)
+                ? a.H32t + ((long)((cell * a.NH + half) * a.kchunks + c) * a.NT) * 32
+                : a.Bext + ((long)(ext0 + c - a.kchunks) * a.NH + half) * a.NT * 32;
+            if (a.dbg & 64) { ptx::bulk_load(dst, src, (uint32_t)bbytes / 2, &full[s]); ptx::bulk_load(dst + bbytes / 2, src, (uint32_t)bbytes / 2, &full[s]); }
+            else ptx::bulk_load(dst, src, (uint32_t)bbytes, &full[s]);
+          }
       }
       __syncwarp();
     } else {
       // ================= MMA issuer =================
       if (lane == 0) {
-        ptx::mbar_wait(accum_empty, (tile_iter & 1) ^ 1);   // accumulators drained by the previous tile's epilogue
-        ptx::tc_fence_after_sync();
-        for (int c = 0; c < nchunks; ++c) {
-          const uint32_t s = (it + c) % a.stages, ph = ((it + c) / a.stages) & 1;
-          ptx::mbar_wait(&full[s], ph);
-          ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes of the A tiles -> tensor-core (async proxy) reads
+        uint32_t itc = it;
+        for (int vt = 0; vt < a.nvt; ++vt) {
+          const uint32_t buf = (sub_iter + vt) & 1, use = (sub_iter + vt) >> 1;
+          ptx::mbar_wait(&accum_empty[buf], (use & 1) ^ 1);   // buffer drained by the epilogue of two subtiles ago
           ptx::tc_fence_after_sync();
-          const uint32_t abase = ptx::smem_u32(smem + s * sbytes), bbase = abase + abytes;
-          const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
-          for (int ks = 0; ks < ksteps; ++ks) {
-            // B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B per K step inside the 128-B row
-            const uint64_t bdesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);
-            for (int j = 0; j < nv; ++j) {
+          const uint32_t dtm = tmem_base + buf * a.acc_stride;
+          for (int c = 0; c < nchunks; ++c, ++itc) {
+            const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
+            ptx::mbar_wait(&full[s], ph);
+            if (!(a.dbg & 32)) ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes of the A tile -> tensor-core (async proxy) reads
+            ptx::tc_fence_after_sync();
+            const uint32_t abase = ptx::smem_u32(smem + s * sbytes), bbase = abase + kABytes;
+            const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
+            for (int ks = 0; ks < ksteps; ++ks) {
               // A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
               // 512 B apart (SBO); one K step = 8 rows = 1024 B
-              const uint64_t adesc = ptx::smem_desc(abase + j * kABytes + ks * 1024, 4096, 512, 1);
-              if (!(a.dbg & 8)) ptx::mma_tf32_ss(tmem_base + (uint32_t)(j * a.NT), adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+              const uint64_t adesc = ptx::smem_desc(abase + ks * 1024, 4096, 512, 1);
+              // B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B per K step inside the 128-B row
+              const uint64_t bdesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);
+              if (!(a.dbg & 8)) ptx::mma_tf32_ss(dtm, adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
             }
+            ptx::mma_commit(&empty[s]);
           }
-          ptx::mma_commit(&empty[s]);
+          ptx::mma_commit(&accum_full[buf]);
         }
-        ptx::mma_commit(accum_full);
       }
       __syncwarp();
     }
-    it += nchunks;
+    it += (uint32_t)(nchunks * a.nvt);
+    sub_iter += (uint32_t)a.nvt;
   }
   __syncthreads();
   if (warp == 9) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
@@ -314,13 +318,13 @@ void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
   *NT = (per + 15) / 16 * 16;
 }
 
-size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 2) * 8 + 16; }
+size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 4) * 8 + 16; }
 int stages_for(int NH, int NT) {
   const size_t budget = 227 * 1024 - 1024;  // dynamic shared memory per CTA, less the alignment slack
-  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(2 * kABytes + NT * 128));
+  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(kABytes + NT * 128));
   return std::min(st, kMaxStages);
 }
-size_t smem_bytes(int NH, int NT) { return (size_t)stages_for(NH, NT) * (2 * kABytes + NT * 128) + smem_fixed(NH, NT); }
+size_t smem_bytes(int NH, int NT) { return (size_t)stages_for(NH, NT) * (kABytes + NT * 128) + smem_fixed(NH, NT); }
 
 TcPlan* get_plan(pawfe_ctx* c) {
   if (c->tc_plan) return (TcPlan*)c->tc_plan;
@@ -359,6 +363,8 @@ TcPlan* get_plan(pawfe_ctx* c) {
 
 }  // namespace
 
+void tc_shape(const pawfe_ctx* c, int* NH, int* NT) { shape_for(c, NH, NT); }
+
 void tc_invalidate(pawfe_ctx* c) {
   if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
 }
@@ -385,31 +391,20 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.kchunks = (c->ldk + kChunkK - 1) / kChunkK;
   a.ksteps_last = (c->ldk - (a.kchunks - 1) * kChunkK) / 8;
   a.nvt = (B + kTileV - 1) / kTileV;
-  a.nvg = (a.nvt + 1) / 2;
-  a.ntiles = c->ncell * a.nvg * a.NH;
+  a.ntiles = c->ncell * a.NH;
   a.stages = stages_for(p->NH, p->NT);
   uint32_t cols = 32;
-  while ((int)cols < std::min(a.nvt, 2) * a.NT) cols <<= 1;
-  a.tmem_cols = cols;
+  while ((int)cols < a.NT) cols <<= 1;
+  a.acc_stride = cols;
+  a.tmem_cols = 2 * cols;
   a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
   a.scale_mode = 0;
+  a.H32t = p->d_H32t; a.Bext = nullptr;
   a.ext_start = nullptr; a.ext_atom = nullptr; a.Wcat = nullptr; a.ldw = 0; a.ext_ksteps = 0;
   if (ext) {
     a.scale_mode = ext->scale_mode;
     if (ext->nchunks > 0) {
-      if (p->ext_ptr != ext->Bext) {
-        EncodeTiledFn enc = get_encode();
-        cuuint64_t dims[2] = {32, (cuuint64_t)ext->nchunks * c->n};
-        cuuint64_t strides[1] = {32 * sizeof(float)};
-        cuuint32_t box[2] = {(cuuint32_t)kChunkK, (cuuint32_t)p->NT};
-        cuuint32_t estr[2] = {1, 1};
-        CUresult r = enc(&p->tmapE, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)ext->Bext, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) { c->err = "tcgen05 cell kernel: K-extension tensor map failed"; return PAWFE_ECUDA; }
-        p->ext_ptr = ext->Bext;
-      }
-      a.ext_start = ext->ext_start; a.ext_atom = ext->ext_atom; a.Wcat = ext->Wcat; a.ldw = ext->ldw;
+      a.ext_start = ext->ext_start; a.ext_atom = ext->ext_atom; a.Wcat = ext->Wcat; a.ldw = ext->ldw; a.Bext = ext->Bext;
       a.ext_ksteps = ext->ksteps;
     }
   }

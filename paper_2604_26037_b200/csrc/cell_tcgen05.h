@@ -3,6 +3,9 @@
 #pragma once
 #include "common.h"
 
+// Split of the n output nodes of a cell into NH halves of NT columns (NT a multiple of 16) used by the kernel.
+void tc_shape(const pawfe_ctx* ctx, int* NH, int* NT);
+
 // Drop any cached tensor maps / plans (called when the cell matrices are rebuilt or freed).
 void tc_invalidate(pawfe_ctx* ctx);
 
@@ -21,7 +24,7 @@ struct TcExt {
   int scale_mode;              // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
   long nchunks;
   const int* ext_start; const int* ext_atom;
-  const float* Bext;
+  const float* Bext;           // [chunk][half][NT][32] floats, rows 128-byte swizzled (api_fused.cu k_build_ext)
   const float* Wcat; long ldw;
   int ksteps;
 };

@@ -140,6 +140,7 @@ struct pawfe_ctx {
   std::vector<double> xi, wgll, K1, M1, G1;  // host 1-D tables
   double* d_md1 = nullptr;     // device: [N0+N1+N2] M_D factors, then [N0+N1+N2] M_D^-1 factors
   MeshDev md{};
+  double* d_M1 = nullptr;      // device: 1-D consistent mass matrix M1 [n1][n1] on the reference interval
   double* d_Mref64 = nullptr;  // reference mass cell matrix M^e (n x n), real
   float* d_Mref32 = nullptr;   // same in FP32 with row stride ldk
 

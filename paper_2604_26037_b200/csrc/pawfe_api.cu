@@ -14,6 +14,7 @@ using namespace pawfe;
 
 void pawfe_free_mesh(pawfe_ctx* c) {
   cudaFree(c->d_md1); c->d_md1 = nullptr;
+  cudaFree(c->d_M1); c->d_M1 = nullptr;
   cudaFree(c->d_Mref64); c->d_Mref64 = nullptr;
   cudaFree(c->d_Mref32); c->d_Mref32 = nullptr;
   c->have_mesh = false;
@@ -155,6 +156,7 @@ extern "C" pawfe_status pawfe_mesh_create(pawfe_ctx* c, const int ncells[3], con
     off += c->N[d];
   }
   TRY(upload(c, &c->d_md1, md));
+  TRY(upload(c, &c->d_M1, c->M1));
   MeshDev& m = c->md;
   off = 0;
   for (int d = 0; d < 3; ++d) {
