@@ -69,7 +69,7 @@ pawfe_status launch_dmma_mt(pawfe_ctx* c, const double* A, long cell_stride, con
     CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     smem_attr = smem;
   }
-  kern<<<dim3(c->ncell, ceil_div(Wr, dmma::kTN)), dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   KERNEL_CHECK(c, "k_cell_dmma");
   return PAWFE_OK;
 }

@@ -57,7 +57,9 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
   unsigned char* stage0 = smem_raw;
   long* nodeJ = reinterpret_cast<long*>(smem_raw + kStages * (aBytes + bBytes));
   const int n = md.n, n1 = md.n1;
-  const int e = blockIdx.x, v0 = blockIdx.y * kTN;
+  // column tile fastest: the CTAs that share a cell matrix are scheduled together and the re-reads hit L2
+  const int ntile = (Wr + kTN - 1) / kTN;
+  const int e = blockIdx.x / ntile, v0 = (blockIdx.x % ntile) * kTN;
   {
     int cx, cy, cz;
     mesh_cell_coords(md, e, &cx, &cy, &cz);
