@@ -268,9 +268,33 @@ def run_own(args):
         # SIMT FMA pipe: 148 SMs x 128 FP32 lanes x 2 flop at the clock seen under load
         mhz = (clocks or {}).get("sm_mhz") or 1965.0
         peak = 148 * 128 * 2 * mhz * 1e6 / 1e12 * (0.5 if prec == FP64 else 1.0)
-        peak_note = "148 SM x 128 lanes x 2 flop x SM clock under load (FP64: half)"
-        bound = "alu"
-    achieved = flops_launch / (cell_avg_ms * 1e-3) / 1e12 if cell_avg_ms > 0 else 0.0
+        peak_note = "148 SM x 128 lanes x 2 flop x SM clock under load (FP64: half, the DMMA / DFMA rate)"
+        bound = "tensor" if "dmma" in kname else "alu"
+    tflops = flops_launch / (cell_avg_ms * 1e-3) / 1e12 if cell_avg_ms > 0 else 0.0
+    # Roofline of the dominant kernel.  The fused tcgen05 step kernel is HBM-bound at these block
+    # widths: algorithmic bytes per launch = H^e stream (4 n^2 N_c, x2 complex) + read R_Y (4 B) +
+    # read-modify-write R_X (8 B) per dof*vec (x2 complex).  Other cell kernels: tensor / ALU flop rate.
+    cw = 2 if cplx else 1
+    bytes_launch = 4.0 * n * n * ncell * cw + 12.0 * M * B * cw
+    gbs = bytes_launch / (cell_avg_ms * 1e-3) / 1e9 if cell_avg_ms > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "cell_kernel_traffic.csv")   # written from the committed ncu capture
+    if os.path.exists(tpath):
+        import csv
+        for row in csv.DictReader(open(tpath)):
+            if row["workload"] == cfg.name and row["kernel"] == kname and row["precision"] == args.prec:
+                traffic = float(row["dram_bytes_per_launch"])
+    if "tcgen05" in kname:
+        roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": gbs / peaks["hbm"], "traffic": traffic, "peak_source": f"{peaks['src']} copy bandwidth",
+                "algorithmic_bytes_per_launch": bytes_launch,
+                "tensor": {"achieved_tflops": tflops, "peak_tflops": peak, "frac": tflops / peak, "peak_source": peak_note}}
+    else:
+        roof = {"kernel": kname, "bound": bound, "achieved": tflops, "peak": peak, "unit": "TFLOP/s",
+                "frac": tflops / peak if peak else None, "traffic": traffic, "peak_source": peak_note}
+    roof.update({"launches": ncell_launch, "avg_ms": cell_avg_ms, "share_of_step": cell_ms / ms})
+    # whole-step HBM view: SURVEY.md 8(d) algorithmic bytes per dof*vec*step of the fully fused step
+    step_bytes = (4.0 * n * n * ncell * cw / (M * B) + 20.0 * cw)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -285,11 +309,10 @@ def run_own(args):
         "e2e": {"value": world * units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nblk * blk_bytes,
                 "d2h_bytes_per_step": nblk * blk_bytes, "steps": e2e_steps},
         "gpu_launches": launches,
-        "roofline": {"kernel": kname, "bound": bound, "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": None,
-                     "launches": ncell_launch, "avg_ms": cell_avg_ms, "share_of_step": cell_ms / ms,
-                     "peak_source": peak_note,
-                     "hbm_stream_gbs": (4.0 * n * n * ncell * (2 if cplx else 1)) / (cell_avg_ms * 1e-3) / 1e9 if cell_avg_ms > 0 else None},
+        "roofline": roof,
+        "step_hbm": {"algorithmic_bytes_per_dof_vec_step": step_bytes,
+                     "achieved_gbs": step_bytes * value / world / 1e9, "peak_gbs": peaks["hbm"],
+                     "frac": step_bytes * value / world / 1e9 / peaks["hbm"]},
     }
     if world == 1 and not args.no_cpu_baseline:
         smp = OracleSample(args.config)

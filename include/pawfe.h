@@ -171,7 +171,7 @@ pawfe_status pawfe_cell_timing(pawfe_ctx* ctx, int enable);
 pawfe_status pawfe_cell_timing_read(pawfe_ctx* ctx, long* launches, double* ms);
 
 /* Name of the cell-contraction kernel variant a given (prec, B) runs ("tcgen05_tf32", "simt_fp32",
- * "simt_fp64", ...).  Static string. */
+ * "dmma_fp64", ...).  Static string. */
 const char* pawfe_cell_kernel_name(const pawfe_ctx* ctx, pawfe_prec prec, int B);
 
 #if defined(__GNUC__)

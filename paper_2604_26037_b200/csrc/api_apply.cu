@@ -138,7 +138,7 @@ pawfe_status pawfe_apply_HS(pawfe_ctx* c, int op, bool tf32, const TX* X, long l
   TRY(zero_block(c, Y, ldy, B));
   const TC* A = op == 0 ? OpData<TC>::H(c) : OpData<TC>::Mref(c);
   long stride = op == 0 ? (long)c->n * OpData<TC>::lda(c) : 0;
-  const bool timed = (op == 0) && sizeof(typename ScalarTraits<TC>::real) == 4;  // the loop's contraction
+  const bool timed = (op == 0) && sizeof(typename ScalarTraits<TC>::real) == sizeof(typename ScalarTraits<TX>::real);  // the loop's contraction
   if (timed) prof_begin(c);
   pawfe_status st;
   if (tf32 && op == 0) st = launch_cell<TX, TY, TC, true>(c, A, stride, OpData<TC>::lda(c), X, ldx, Y, ldy, B, 0, 1.0);
@@ -237,7 +237,7 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
 
 extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec prec, int B) {
   if (!c) return "none";
-  if (prec == PAWFE_FP64) return "simt_fp64";
+  if (prec == PAWFE_FP64) return "dmma_fp64";
   if (prec == PAWFE_FP32) return "simt_fp32";
   if (!c->cplx && tc_supported(c, B)) return "tcgen05_tf32";
   return "simt_tf32_emulated";

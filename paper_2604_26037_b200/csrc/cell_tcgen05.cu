@@ -2,21 +2,21 @@
 // with extraction (step i, L343) and assembly (step iv, L347), on tcgen05 tensor cores in TF32 with FP32
 // accumulation in tensor memory (TF32: L11, L27; FP32 storage: L374).
 //
-// Formulation.  Per cell e and per tile of 128 vectors the kernel computes the TRANSPOSED product
-//     Y_e^T (128 vec x n) = X_e^T (128 vec x n) * H^e^T (n x n)
+// Formulation.  Per cell e, node half and tile of 128 vectors the kernel computes the TRANSPOSED product
+//     Y_e^T (128 vec x NT) = X_e^T (128 vec x n) * H^e^T (n x NT)
 // so that the MMA M dimension (128 TMEM lanes) is the vector index and the N dimension the output node:
-//   * operand A = X_e^T is "MN-major": a K-chunk is 32 gathered node rows of 128 contiguous vectors, exactly the
-//     shape of the global [dof][vec] block, copied by cp.async into the canonical 128-byte-swizzled layout;
-//   * operand B = H^e is "K-major": rows of the row-major cell matrix, streamed by TMA (2-D tiled map, 128-byte
-//     swizzle) -- each cell matrix is read once per (vector tile, node half);
-//   * the accumulator (128 lanes x NT columns) is read back lane = vector, so one warp-wide reduction per node
-//     writes 32 consecutive vectors = one coalesced 128-byte segment of the global row.
-// n = (p+1)^3 output nodes are split into NH = 1 or 2 halves of NT <= 256 columns (NT a multiple of 16) so that
-// two CTAs fit one SM (2 x 256 TMEM columns, 2 x <= 110 KB shared memory): while one CTA drains its accumulator
-// the other one runs its MMAs.  Persistent CTAs loop over (cell, vector tile, node half) tiles.
+//   * operand A = X_e^T is "MN-major": a K chunk is 32 gathered node rows of 128 contiguous vectors, exactly the
+//     shape of the global [dof][vec] block, copied by cp.async into the 128-byte-swizzle / 32-byte-atom layout;
+//   * operand B = H^e is "K-major": stored re-tiled and pre-swizzled ([cell][half][K chunk][NT][32 floats]) so that
+//     each chunk is ONE contiguous cp.async.bulk copy that lands in the SW128 K-major layout;
+//   * the accumulator (128 lanes x NT columns) is read back lane = vector, transposed through shared memory and
+//     added to the global rows with 16-byte vector reductions (4 vectors of one node per thread).
+// n = (p+1)^3 output nodes are split into NH = 1 or 2 halves of NT <= 256 columns (NT a multiple of 16).  Optional
+// K-extension chunks (fused.h) append low-rank projector terms to the same accumulation.
 //
-// Warp roles (192 threads): warps 0-3 gather producers, then epilogue; warp 4 TMA producer; warp 5 TMEM owner and
-// MMA issuer.  Pipelines: full[s] / empty[s] per shared-memory stage, accum for the accumulator.
+// One persistent CTA per SM, 10 warps: 0-3 epilogue, 4-7 gather producers, 8 bulk-copy producer, 9 MMA issuer and
+// TMEM owner.  Pipelines: full[s] / empty[s] per shared-memory stage, accum_full[b] / accum_empty[b] per
+// accumulator buffer (two buffers: the epilogue of one vector tile runs under the MMAs of the next).
 #include "cell_tcgen05.h"
 #include "ptx_sm100.cuh"
 #include <cstdio>

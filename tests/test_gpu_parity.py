@@ -162,3 +162,71 @@ def test_col_norms():
         ctx.col_norms(prec, Xd, B, B, out)
         torch.cuda.synchronize()
         assert np.allclose(out.cpu().numpy(), want, rtol=1e-6 if name == "fp32" else 1e-13)
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json configs[1] at FULL size, in the launch configuration bench.py times (B = 200, TF32 mode)
+# ------------------------------------------------------------------------------------------------
+_FULL = {}
+
+
+def _full_cfg1():
+    if "ctx" not in _FULL:
+        if not torch.cuda.is_available():
+            pytest.skip("no CUDA device")
+        from paper_2604_26037_b200 import context_from_system
+        cfg = get_config(1)
+        sysd = make_system(cfg)
+        _FULL["cfg"], _FULL["sys"] = cfg, sysd
+        _FULL["ctx"] = context_from_system(sysd, device=0, stream=torch.cuda.current_stream().cuda_stream)
+    return _FULL["cfg"], _FULL["sys"], _FULL["ctx"]
+
+
+def test_full_size_cfg1_H_sampled_rows():
+    """H X at 884,736 dofs x 200 vectors (tcgen05 kernel, two vector tiles, K-extension) against the oracle's
+    row-by-row evaluation (oracle.operators.apply_H_rows) on the nodes of two sampled cells."""
+    from oracle.operators import apply_H_rows
+    from paper_2604_26037_b200 import TF32, FP64
+    cfg, sysd, ctx = _full_cfg1()
+    B = cfg.block
+    X = random_block(cfg, B, stream=11)
+    cells = [(0, 0, 0), (7, 15, 3)]          # a corner cell (periodic wrap) and an interior one
+    want = apply_H_rows(sysd, X, cells)
+    for prec, name, tol in ((TF32, "tf32", TOL["tf32"]), (FP64, "fp64", TOL["fp64"])):
+        Xd = _to_dev(X, name, False)
+        Yd = torch.empty_like(Xd)
+        ctx.apply_H(prec, Xd, Yd, B, B)
+        torch.cuda.synchronize()
+        for J, ref in want:
+            got = Yd[torch.from_numpy(np.asarray(J)).cuda()].cpu().numpy().astype(np.float64)
+            assert _relerr(got, ref) < tol, (name, _relerr(got, ref))
+
+
+def test_full_size_cfg1_filter_properties():
+    """Properties of one full-size TF32 filter call that hold at any size: (i) columns are filtered independently, so
+    a 64-column call reproduces the first 64 columns of the 200-column call (different tile shapes, ragged tail);
+    (ii) the output is finite and (iii) scaling the input block scales the output (linearity in X for fixed Lambda)."""
+    from paper_2604_26037_b200 import TF32
+    from paper_2604_26037_b200.harness import Harness
+    cfg, sysd, ctx = _full_cfg1()
+    B, m = cfg.block, 6
+    M = ctx.num_dofs()
+    hz = Harness(ctx, M, False)
+    gen = torch.Generator(device="cuda").manual_seed(cfg.seed)
+    X0 = torch.rand((M, B), dtype=torch.float64, device="cuda", generator=gen) - 0.5
+    X, lam = hz.rayleigh_ritz(hz.s_orthonormalise(X0))
+    bU = hz.upper_bound(k=10, seed=1)
+    b0, bW = float(lam[0]) - 0.1, 0.5 * (float(lam[0]) - 0.1 + bU)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    A = X.to(torch.float32).contiguous()
+    ctx.cheb_filter(TF32, m, b0, bW, bU, A, lam, B, B, ws, nbytes)
+    Bsub = X[:, :64].to(torch.float32).contiguous()
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Bsub, lam[:64], 64, 64, ws, nbytes)
+    C2 = (2.0 * X).to(torch.float32).contiguous()
+    ctx.cheb_filter(TF32, m, b0, bW, bU, C2, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(A).all())
+    nrm = A[:, :64].double().norm()
+    assert float((A[:, :64].double() - Bsub.double()).norm() / nrm) < 1e-4
+    assert float((C2.double() - 2.0 * A.double()).norm() / (2.0 * A.double().norm())) < 1e-4
