@@ -159,6 +159,11 @@ extern "C" pawfe_status pawfe_filter_workspace(pawfe_ctx* c, pawfe_prec prec, in
   size_t cw = c->cplx ? 2 : 1;
   size_t ss = (prec == PAWFE_FP64 ? 8 : 4) * cw, sd = 8 * cw;
   *bytes = ws_layout(c->M, B, ss, sd).total;
+  if (fused_supported(c, prec, B)) {
+    // fused step (fused.h): Yt (FP64) + Rt_X + Rt_Y (FP32); S X, T and H T are never stored
+    const size_t ldw = ((size_t)B + 3) / 4 * 4;
+    *bytes = align256((size_t)c->M * ldw * 8) + 2 * align256((size_t)c->M * ldw * 4);
+  }
   return PAWFE_OK;
 }
 

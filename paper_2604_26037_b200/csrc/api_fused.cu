@@ -630,11 +630,9 @@ pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const doub
   const size_t blk_s = ((size_t)c->M * ldw * 4 + 255) / 256 * 256, blk_d = ((size_t)c->M * ldw * 8 + 255) / 256 * 256;
   char* ws = (char*)workspace;
   double* Yt = (double*)ws;
-  double* SX = (double*)(ws + blk_d);
-  float* RX = (float*)(ws + 2 * blk_d);
-  float* RY = (float*)(ws + 2 * blk_d + blk_s);
+  float* RX = (float*)(ws + blk_d);
+  float* RY = (float*)(ws + blk_d + blk_s);
   // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda, fused (setup_fp64.cuh): S X is never stored ----
-  (void)SX;
   CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
   TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
   {

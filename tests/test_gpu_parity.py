@@ -230,3 +230,24 @@ def test_full_size_cfg1_filter_properties():
     nrm = A[:, :64].double().norm()
     assert float((A[:, :64].double() - Bsub.double()).norm() / nrm) < 1e-4
     assert float((C2.double() - 2.0 * A.double()).norm() / (2.0 * A.double().norm())) < 1e-4
+
+
+@pytest.mark.parametrize("B", [10, 130])
+def test_filter_ragged_block_width(B):
+    """Block widths that are not a multiple of 4 (config 2 has B = 250) or just over one vector tile: the workspace
+    rows are padded to a multiple of 4 and the pad columns must stay inert."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import TF32
+    cfg, sysd, ops, ctx = _setup("cfg1_twin")
+    m = 5
+    X0 = random_block(cfg, B, stream=21) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+    Xd = _to_dev(X, "tf32", False)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, False), want) < 5e-2
