@@ -221,7 +221,18 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
     return pawfe_apply_HS<double, double, double>(c, 0, false, (const double*)X, ldx, (double*)Y, ldy, B);
   }
   bool tf32 = prec == PAWFE_TF32;
-  if (c->cplx) return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
+  if (c->cplx) {
+    if (tf32 && tc_usable(c, X, 2 * ldx, Y, 2 * ldy, 2 * B)) {
+      // complex TF32: interleaved (re, im) columns as a real block of 2B columns; P / Q accumulators in the kernel
+      TRY(zero_block(c, (float2*)Y, ldy, B));
+      prof_begin(c);
+      pawfe_status st = tc_cell_apply(c, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, 2 * B, 1.0f);
+      prof_end(c);
+      TRY(st);
+      return pawfe_apply_nonlocal<float2, float2, float2>(c, OpData<float2>::D(c), 1.0, (const float2*)X, ldx, 0, (float2*)Y, ldy, 0, B);
+    }
+    return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
+  }
   if (tf32 && tc_usable(c, X, ldx, Y, ldy, B) && fused_supported(c, prec, B))
     return fused_apply_H(c, (const float*)X, ldx, (float*)Y, ldy, B);
   if (tf32 && tc_usable(c, X, ldx, Y, ldy, B)) {
@@ -239,7 +250,7 @@ extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec pre
   if (!c) return "none";
   if (prec == PAWFE_FP64) return "dmma_fp64";
   if (prec == PAWFE_FP32) return "simt_fp32";
-  if (!c->cplx && tc_supported(c, B)) return "tcgen05_tf32";
+  if (tc_supported(c, B)) return "tcgen05_tf32";
   return "simt_tf32_emulated";
 }
 

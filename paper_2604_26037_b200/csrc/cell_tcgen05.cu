@@ -40,6 +40,7 @@ struct TcArgs {
   int nvt;       // vector tiles of 128 in the block (processed one after the other inside a tile)
   int ntiles;    // ncell * NH
   int stages;
+  int ncomp;     // 1: real cell matrices; 2: complex (two B blocks Re, Im and two accumulators P, Q per buffer)
   uint32_t tmem_cols, acc_stride, idesc;   // two accumulators of NT columns, acc_stride apart
   int scale_mode;            // 0: Y += alpha * acc;  1: Y += alpha * M_D^-1[J] * acc
   // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
@@ -49,9 +50,6 @@ struct TcArgs {
 };
 
 struct TcPlan {
-  CUtensorMap tmapH;
-  CUtensorMap tmapE;             // K-extension blocks [chunk * n + I][32], built on first use for ext_ptr
-  const void* ext_ptr = nullptr;
   float* d_H32t = nullptr;       // cell matrices re-tiled for streaming: [cell][half][K chunk][NT rows][32] floats
   int NT = 0, NH = 0;
   bool ok = false;
@@ -60,12 +58,13 @@ struct TcPlan {
 // Re-tile the row-major FP32 cell matrices so that every (cell, half, K chunk) block the kernel loads is one
 // contiguous NT x 128-byte region of HBM (row-major [cell][n][ldk] gives NT scattered 128-byte pieces per load,
 // which costs DRAM page locality).  Rows >= n and columns >= n are zero.
-__global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH, int NT, int kchunks, long total,
-                             float* __restrict__ out) {
+__global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH, int NT, int kchunks, int ncomp,
+                             long total, float* __restrict__ out) {
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
     const int kk = (int)(i & 31);
     long t = i >> 5;
     const int r = (int)(t % NT); t /= NT;
+    const int comp = (int)(t % ncomp); t /= ncomp;   // complex: [chunk][Re block][Im block]
     const int ch = (int)(t % kchunks); t /= kchunks;
     const int half = (int)(t % NH);
     const long cell = t / NH;
@@ -73,7 +72,7 @@ __global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH
     // 128-byte-swizzled image: 16-byte piece j of row r is stored at piece j ^ (r % 8), so that a plain contiguous
     // bulk copy of the block lands in shared memory in the layout the K-major SW128 matrix descriptor expects
     const long o = (i & ~31L) + ((((kk >> 2) ^ (r & 7)) << 2) | (kk & 3));
-    out[o] = (I < n && k < n) ? H[(cell * n + I) * ldk + k] : 0.f;
+    out[o] = (I < n && k < n) ? H[((cell * n + I) * ldk + k) * ncomp + comp] : 0.f;
   }
 }
 
@@ -84,10 +83,11 @@ __device__ __forceinline__ void bar_sync_128(int id) { asm volatile("bar.sync %0
 // from L2.  Accumulators are double-buffered in tensor memory (subtile parity), so the assembly epilogue of one
 // subtile runs under the loads and MMAs of the next.  Roles are decoupled through mbarriers only.
 __global__ void __launch_bounds__(kThreads, 1)
-k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant__ CUtensorMap tmapE, const TcArgs a) {
+k_cell_tcgen05(const TcArgs a) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  const int bbytes = a.NT * 128;
-  const int sbytes = kABytes + bbytes;                  // one stage: [A][B]
+  const int bbytes1 = a.NT * 128;                       // one matrix block (Re or Im)
+  const int bbytes = a.ncomp * bbytes1;
+  const int sbytes = kABytes + bbytes;                  // one stage: [A][B (Re)][B (Im)]
   long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows: byte offset or -1
   long* eJ = gJ + a.NH * a.NT;                                            // [NT] output rows of this half
   float* eS = reinterpret_cast<float*>(eJ + a.NT);                        // [NT] output scale
@@ -104,7 +104,6 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
     for (int b = 0; b < 2; ++b) { ptx::mbar_init(&accum_full[b], 1); ptx::mbar_init(&accum_empty[b], 128); }
     ptx::fence_barrier_init();
   }
-  if (warp == 8 && lane == 0) { ptx::prefetch_tmap(&tmapH); if (a.ext_start) ptx::prefetch_tmap(&tmapE); }
   if (warp == 9) ptx::tmem_alloc(tmem_slot, a.tmem_cols);
   ptx::tc_fence_before_sync();
   __syncthreads();
@@ -152,7 +151,41 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
         const int vb = vt * kTileV + warp * 32;
         const bool vok = vb + v4 < a.B;             // B % 4 == 0: a float4 is all in or all out
         char* yv = reinterpret_cast<char*>(a.Y + vb + v4);
-        if (vb < a.B && !(a.dbg & 16)) {
+        if (vb < a.B && !(a.dbg & 16) && a.ncomp == 2) {
+          // complex: columns are interleaved (re, im); with P = X^T Hr^T and Q = X^T Hi^T,
+          //   Y_re = P_re - Q_im,  Y_im = P_im + Q_re  ->  y = P + (lane odd ? +1 : -1) * Q of the partner lane
+          const float sg = (lane & 1) ? 1.f : -1.f;
+          for (int col0 = 0; col0 < ncols; col0 += 16) {
+            uint32_t r[16], q[16];
+            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
+            ptx::tmem_ld16(taddr, r);
+            ptx::tmem_ld16(taddr + a.NT, q);
+            ptx::tmem_ld_wait();
+            const int nq = min(16, ncols - col0);
+#pragma unroll
+            for (int k = 0; k < 16; k += 4) {
+              const float4 sc = *reinterpret_cast<const float4*>(&eS[col0 + k]);
+              const float scs[4] = {sc.x, sc.y, sc.z, sc.w};
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const float qp = __shfl_xor_sync(0xffffffffu, __uint_as_float(q[k + u]), 1);
+                stg[(k + u) * 32 + lane] = scs[u] * fmaf(sg, qp, __uint_as_float(r[k + u]));
+              }
+            }
+            __syncwarp();
+            if (vok) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const int k = sub + 4 * i;
+                if (k < nq) {
+                  const long off = eJ[col0 + k];
+                  if (off >= 0) ptx::red_add_v4(reinterpret_cast<float*>(yv + off), *reinterpret_cast<const float4*>(&stg[k * 32 + v4]));
+                }
+              }
+            }
+            __syncwarp();
+          }
+        } else if (vb < a.B && !(a.dbg & 16)) {
           for (int col0 = 0; col0 < ncols; col0 += 32) {
             uint32_t r[32];
             const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
@@ -251,7 +284,7 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
             const uint32_t dst = ptx::smem_u32(smem + s * sbytes + kABytes);
             // both operand streams are stored pre-swizzled and block-contiguous: one linear bulk copy per chunk
             const float* src = (c < a.kchunks)
-                ? a.H32t + ((long)((cell * a.NH + half) * a.kchunks + c) * a.NT) * 32
+                ? a.H32t + ((long)((cell * a.NH + half) * a.kchunks + c) * a.NT) * 32 * a.ncomp
                 : a.Bext + ((long)(ext0 + c - a.kchunks) * a.NH + half) * a.NT * 32;
             if (a.dbg & 64) { ptx::bulk_load(dst, src, (uint32_t)bbytes / 2, &full[s]); ptx::bulk_load(dst + bbytes / 2, src, (uint32_t)bbytes / 2, &full[s]); }
             else ptx::bulk_load(dst, src, (uint32_t)bbytes, &full[s]);
@@ -281,6 +314,10 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
               // B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B per K step inside the 128-B row
               const uint64_t bdesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);
               if (!(a.dbg & 8)) ptx::mma_tf32_ss(dtm, adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+              if (a.ncomp == 2) {
+                const uint64_t bdesc2 = ptx::smem_desc_sw128(bbase + bbytes1 + ks * 32, 16, 1024);
+                ptx::mma_tf32_ss(dtm + (uint32_t)a.NT, adesc, bdesc2, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+              }
             }
             ptx::mma_commit(&empty[s]);
           }
@@ -296,60 +333,41 @@ k_cell_tcgen05(const __grid_constant__ CUtensorMap tmapH, const __grid_constant_
   if (warp == 9) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-        q == cudaDriverEntryPointSuccess)
-      fn = (EncodeTiledFn)p;
-  }
-  return fn;
-}
-
 void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
-  *NH = c->n > 256 ? 2 : 1;
+  // two accumulator buffers of ncomp * NT columns must fit the 512 TMEM columns
+  const int maxnt = c->cplx ? 128 : 256;
+  *NH = (c->n + maxnt - 1) / maxnt;
   int per = (c->n + *NH - 1) / *NH;
   *NT = (per + 15) / 16 * 16;
 }
 
-size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 4) * 8 + 16; }
-int stages_for(int NH, int NT) {
+size_t smem_fixed_(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 4) * 8 + 16; }
+size_t smem_fixed(int NH, int NT) { return smem_fixed_(NH, NT); }
+int stages_for(int NH, int NT, int ncomp) {
   const size_t budget = 227 * 1024 - 1024;  // dynamic shared memory per CTA, less the alignment slack
-  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(kABytes + NT * 128));
+  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(kABytes + ncomp * NT * 128));
   return std::min(st, kMaxStages);
 }
-size_t smem_bytes(int NH, int NT) { return (size_t)stages_for(NH, NT) * (kABytes + NT * 128) + smem_fixed(NH, NT); }
+size_t smem_bytes(int NH, int NT, int ncomp) {
+  return (size_t)stages_for(NH, NT, ncomp) * (kABytes + ncomp * NT * 128) + smem_fixed(NH, NT);
+}
 
 TcPlan* get_plan(pawfe_ctx* c) {
   if (c->tc_plan) return (TcPlan*)c->tc_plan;
   TcPlan* p = new TcPlan();
   c->tc_plan = p;
   shape_for(c, &p->NH, &p->NT);
-  EncodeTiledFn enc = get_encode();
-  if (!enc || !c->d_H32) return p;
+  if (!c->d_H32) return p;
+  const int ncomp = c->cplx ? 2 : 1;
   const int kchunks = (c->ldk + kChunkK - 1) / kChunkK;
-  const long rows = (long)c->ncell * p->NH * kchunks * p->NT;
-  if (cudaMalloc((void**)&p->d_H32t, (size_t)rows * 32 * sizeof(float)) != cudaSuccess) { cudaGetLastError(); p->d_H32t = nullptr; return p; }
-  k_retile_h32<<<8 * c->sm_count, 256, 0, c->stream>>>((const float*)c->d_H32, c->n, c->ldk, p->NH, p->NT, kchunks, rows * 32, p->d_H32t);
+  const long elems = (long)c->ncell * p->NH * kchunks * ncomp * p->NT * 32;
+  if (cudaMalloc((void**)&p->d_H32t, (size_t)elems * sizeof(float)) != cudaSuccess) { cudaGetLastError(); p->d_H32t = nullptr; return p; }
+  k_retile_h32<<<8 * c->sm_count, 256, 0, c->stream>>>((const float*)c->d_H32, c->n, c->ldk, p->NH, p->NT, kchunks, ncomp, elems, p->d_H32t);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) return p;
-  cuuint64_t dims[2] = {32, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {32 * sizeof(float)};
-  cuuint32_t box[2] = {(cuuint32_t)kChunkK, (cuuint32_t)p->NT};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = enc(&p->tmapH, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d_H32t, dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return p;
   // the attribute is per function, not per context: only ever raise it
   static size_t smem_attr = 0;
-  size_t smem = smem_bytes(p->NH, p->NT);
+  size_t smem = smem_bytes(p->NH, p->NT, ncomp);
   if (smem > smem_attr) {
     if (cudaFuncSetAttribute(k_cell_tcgen05, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
       cudaGetLastError();
@@ -370,7 +388,7 @@ void tc_invalidate(pawfe_ctx* c) {
 }
 
 bool tc_supported(const pawfe_ctx* c, int B) {
-  if (c->cplx || !c->have_pot || B < 1) return false;
+  if (!c->have_pot || B < 1) return false;
   if (c->n < 16) return false;
   return true;
 }
@@ -381,6 +399,7 @@ bool tc_usable(pawfe_ctx* c, const void* X, long ldx, const void* Y, long ldy, i
   return get_plan(c)->ok;
 }
 
+// Complex contexts: X, Y are the interleaved (re, im) blocks seen as real blocks, B = 2 x vectors, ldx / ldy in floats.
 pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B, float alpha,
                            const TcExt* ext) {
   TcPlan* p = get_plan(c);
@@ -392,9 +411,10 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.ksteps_last = (c->ldk - (a.kchunks - 1) * kChunkK) / 8;
   a.nvt = (B + kTileV - 1) / kTileV;
   a.ntiles = c->ncell * a.NH;
-  a.stages = stages_for(p->NH, p->NT);
+  a.ncomp = c->cplx ? 2 : 1;
+  a.stages = stages_for(p->NH, p->NT, a.ncomp);
   uint32_t cols = 32;
-  while ((int)cols < a.NT) cols <<= 1;
+  while ((int)cols < a.ncomp * a.NT) cols <<= 1;
   a.acc_stride = cols;
   a.tmem_cols = 2 * cols;
   a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
@@ -410,7 +430,7 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   }
   { const char* d = getenv("PAWFE_TC_DBG"); a.dbg = d ? atoi(d) : 0; }
   int grid = std::min(a.ntiles, c->sm_count);
-  k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT), c->stream>>>(p->tmapH, a.ext_start ? p->tmapE : p->tmapH, a);
+  k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT, a.ncomp), c->stream>>>(a);
   KERNEL_CHECK(c, "k_cell_tcgen05");
   return PAWFE_OK;
 }
