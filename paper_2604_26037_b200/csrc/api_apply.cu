@@ -6,10 +6,12 @@
 #include "kernels_simt.cuh"
 #include "kernels_stream.cuh"
 #include "cell_dmma.cuh"
+#include "nonlocal_f32.cuh"
 #include "api_internal.h"
 #include "apply_impl.h"
 #include "fused.h"
 #include <algorithm>
+#include <type_traits>
 
 namespace {
 
@@ -110,6 +112,50 @@ pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, c
   }
 }
 
+// Fast FP32-storage non-local path (nonlocal_f32.cuh): real or complex interleaved blocks as Wr = B * cw real columns.
+template <int NPJ, bool CPLX>
+pawfe_status nonlocal_f32_t(pawfe_ctx* c, const float* Delta, double scale, const float* X, long ldx, int in_scale,
+                            float* Y, long ldy, int out_scale, int B) {
+  constexpr int cw = CPLX ? 2 : 1;
+  typedef typename std::conditional<CPLX, float2, float>::type TC;
+  const int n = c->n, Wr = B * cw;
+  float* P = (float*)c->d_P;
+  float* W = P + (size_t)c->natoms * NPJ * Wr;
+  CUDA_TRY(c, cudaMemsetAsync(P, 0, (size_t)c->natoms * NPJ * Wr * sizeof(float), c->stream));
+  dim3 grid((unsigned)c->npairs, ceil_div(Wr, 128));
+  const size_t head = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16;
+  {
+    const size_t smem = head + ((size_t)NPJ * n * cw + 3) / 4 * 16 + (size_t)NPJ * 128 * 4;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_projF<NPJ, CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_projF<NPJ, CPLX><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx * cw, Wr,
+                                                      in_scale, P, (long)Wr);
+    KERNEL_CHECK(c, "k_projF");
+  }
+  k_coupling<TC><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>((const TC*)Delta, NPJ, (const TC*)P, B, B, scale, (TC*)W);
+  KERNEL_CHECK(c, "k_coupling");
+  {
+    const size_t smem = head + ((size_t)NPJ * n * cw + 3) / 4 * 16;
+    static size_t smem_attr = 0;
+    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatterF<NPJ, CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    k_scatterF<NPJ, CPLX><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, W, (long)Wr, Wr,
+                                                         out_scale, Y, ldy * cw);
+    KERNEL_CHECK(c, "k_scatterF");
+  }
+  return PAWFE_OK;
+}
+template <bool CPLX>
+pawfe_status nonlocal_f32(pawfe_ctx* c, const float* Delta, double scale, const float* X, long ldx, int in_scale, float* Y,
+                          long ldy, int out_scale, int B) {
+  switch (c->npj) {
+#define CASE_NL(N) case N: return nonlocal_f32_t<N, CPLX>(c, Delta, scale, X, ldx, in_scale, Y, ldy, out_scale, B);
+    CASE_NL(1) CASE_NL(2) CASE_NL(3) CASE_NL(4) CASE_NL(5) CASE_NL(6) CASE_NL(7) CASE_NL(8)
+    CASE_NL(9) CASE_NL(10) CASE_NL(11) CASE_NL(12) CASE_NL(13) CASE_NL(14) CASE_NL(15) CASE_NL(16)
+#undef CASE_NL
+  }
+  return PAWFE_EINVAL;
+}
+
 }  // namespace
 
 // Y (+)= nonlocal part:  Y += out_scale o C (scale * Delta (C^dagger (in_scale o X)))
@@ -118,6 +164,13 @@ pawfe_status pawfe_apply_nonlocal(pawfe_ctx* c, const TC* Delta, double scale, c
                                   TY* Y, long ldy, int out_scale, int B) {
   if (c->npairs == 0) return PAWFE_OK;
   TRY(pawfe_ensure_P(c, B));
+  if constexpr (std::is_same<TX, TC>::value && std::is_same<TY, TC>::value &&
+                (std::is_same<TC, float>::value || std::is_same<TC, float2>::value)) {
+    constexpr int cw = ScalarTraits<TC>::cplx ? 2 : 1;
+    // 16-byte pieces: rows and the block width must be multiples of 4 floats
+    if (((ldx * cw) & 3) == 0 && ((ldy * cw) & 3) == 0 && ((B * cw) & 3) == 0 && ((uintptr_t)X & 15) == 0 && ((uintptr_t)Y & 15) == 0)
+      return nonlocal_f32<ScalarTraits<TC>::cplx>(c, (const float*)Delta, scale, (const float*)X, ldx, in_scale, (float*)Y, ldy, out_scale, B);
+  }
   TC* P = (TC*)c->d_P;
   TC* W = P + (size_t)c->natoms * c->npj * B;
   size_t smem = (size_t)c->n * 16 + 4 * PAWFE_MAX_NPJ * 32 * sizeof(TC);
