@@ -7,6 +7,7 @@
 #include "kernels_stream.cuh"
 #include "cell_dmma.cuh"
 #include "nonlocal_f32.cuh"
+#include "setup_fp64.cuh"
 #include "api_internal.h"
 #include "apply_impl.h"
 #include "fused.h"
@@ -161,14 +162,14 @@ pawfe_status nonlocal_f32(pawfe_ctx* c, const float* Delta, double scale, const 
 // Y (+)= nonlocal part:  Y += out_scale o C (scale * Delta (C^dagger (in_scale o X)))
 template <typename TX, typename TY, typename TC>
 pawfe_status pawfe_apply_nonlocal(pawfe_ctx* c, const TC* Delta, double scale, const TX* X, long ldx, int in_scale,
-                                  TY* Y, long ldy, int out_scale, int B) {
+                                  TY* Y, long ldy, int out_scale, int B, const double* colscale) {
   if (c->npairs == 0) return PAWFE_OK;
   TRY(pawfe_ensure_P(c, B));
   if constexpr (std::is_same<TX, TC>::value && std::is_same<TY, TC>::value &&
                 (std::is_same<TC, float>::value || std::is_same<TC, float2>::value)) {
     constexpr int cw = ScalarTraits<TC>::cplx ? 2 : 1;
     // 16-byte pieces: rows and the block width must be multiples of 4 floats
-    if (((ldx * cw) & 3) == 0 && ((ldy * cw) & 3) == 0 && ((B * cw) & 3) == 0 && ((uintptr_t)X & 15) == 0 && ((uintptr_t)Y & 15) == 0)
+    if (!colscale && ((ldx * cw) & 3) == 0 && ((ldy * cw) & 3) == 0 && ((B * cw) & 3) == 0 && ((uintptr_t)X & 15) == 0 && ((uintptr_t)Y & 15) == 0)
       return nonlocal_f32<ScalarTraits<TC>::cplx>(c, (const float*)Delta, scale, (const float*)X, ldx, in_scale, (float*)Y, ldy, out_scale, B);
   }
   TC* P = (TC*)c->d_P;
@@ -177,7 +178,7 @@ pawfe_status pawfe_apply_nonlocal(pawfe_ctx* c, const TC* Delta, double scale, c
   k_proj<TX, TC><<<dim3(c->natoms, ceil_div(B, 32)), 128, smem, c->stream>>>(
       c->md, 0, c->d_atom_pair_start, c->d_pair_cell, OpData<TC>::Cd(c), c->npj, X, ldx, B, in_scale, P, B);
   KERNEL_CHECK(c, "k_proj");
-  k_coupling<TC><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(Delta, c->npj, P, B, B, scale, W);
+  k_coupling<TC><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(Delta, c->npj, P, B, B, scale, W, colscale);
   KERNEL_CHECK(c, "k_coupling");
   k_nl_scatter<TY, TC><<<dim3((unsigned)c->npairs, ceil_div(B, 32)), 128, 0, c->stream>>>(
       c->md, 0, c->d_pair_cell, c->d_pair_atom, OpData<TC>::Cd(c), c->npj, W, B, B, out_scale, Y, ldy);
@@ -199,7 +200,7 @@ pawfe_status pawfe_apply_HS(pawfe_ctx* c, int op, bool tf32, const TX* X, long l
   if (timed) prof_end(c);
   TRY(st);
   const TC* Delta = op == 0 ? OpData<TC>::D(c) : OpData<TC>::dS(c);
-  return pawfe_apply_nonlocal<TX, TY, TC>(c, Delta, 1.0, X, ldx, 0, Y, ldy, 0, B);
+  return pawfe_apply_nonlocal<TX, TY, TC>(c, Delta, 1.0, X, ldx, 0, Y, ldy, 0, B, nullptr);
 }
 
 // Y = S^-1approx X = M_D^-1 X - M_D^-1 C Delta_Sinv C^dagger M_D^-1 X   (Eq. 28)
@@ -208,9 +209,16 @@ pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, l
   typedef typename ScalarTraits<TX>::real RX;
   typedef typename ScalarTraits<TY>::real RY;
   const int cw = ScalarTraits<TX>::cplx ? 2 : 1;
+  if constexpr (std::is_same<RX, float>::value && std::is_same<RY, float>::value) {
+    if (((ldx * cw) & 3) == 0 && ((ldy * cw) & 3) == 0 && ((B * cw) & 3) == 0 && ((uintptr_t)X & 15) == 0 && ((uintptr_t)Y & 15) == 0) {
+      k_scale_mdinv_f4<<<8 * c->sm_count, 256, 0, c->stream>>>(c->md, (const float4*)X, ldx * cw / 4, (float4*)Y, ldy * cw / 4, B * cw / 4);
+      KERNEL_CHECK(c, "k_scale_mdinv_f4");
+      return pawfe_apply_nonlocal<TX, TY, TC>(c, OpData<TC>::dSinv(c), -1.0, X, ldx, 1, Y, ldy, 1, B, nullptr);
+    }
+  }
   k_scale_mdinv<RX, RY><<<4 * c->sm_count, 256, 0, c->stream>>>(c->md, (const RX*)X, ldx * cw, (RY*)Y, ldy * cw, B * cw);
   KERNEL_CHECK(c, "k_scale_mdinv");
-  return pawfe_apply_nonlocal<TX, TY, TC>(c, OpData<TC>::dSinv(c), -1.0, X, ldx, 1, Y, ldy, 1, B);
+  return pawfe_apply_nonlocal<TX, TY, TC>(c, OpData<TC>::dSinv(c), -1.0, X, ldx, 1, Y, ldy, 1, B, nullptr);
 }
 
 template <typename RX>
@@ -219,6 +227,27 @@ pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double
 }
 template pawfe_status pawfe_cell_product_fp64<float>(pawfe_ctx*, const float*, long, double*, long, int);
 template pawfe_status pawfe_cell_product_fp64<double>(pawfe_ctx*, const double*, long, double*, long, int);
+
+// Y -= (S X) Lambda, S = M + C dS C^dagger (Eq. 16), FP64, without storing S X: the mass part by three 1-D sweeps of
+// M^e = (hx hy hz / 8) M1 (x) M1 (x) M1 (setup_fp64.cuh: k_mass_sf), the non-local part with the Ritz value folded into
+// the coupling.  neg_lam / lam: device, [B] doubles (-Lambda and Lambda).  Y: FP64 block with leading dimension ldy.
+template <typename TX, typename TD>
+pawfe_status pawfe_sub_SX_lambda(pawfe_ctx* c, const TX* X, long ldx, TD* Y, long ldy, int B, const double* lam,
+                                 const double* neg_lam) {
+  typedef typename ScalarTraits<TX>::real RX;
+  constexpr int cw = ScalarTraits<TX>::cplx ? 2 : 1;
+  const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
+  static size_t smem_attr = 0;
+  if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_mass_sf<RX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+  k_mass_sf<RX><<<dim3(c->ncell, ceil_div(B * cw, 32)), 256, smem, c->stream>>>(
+      c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, (const RX*)X, ldx * cw, (double*)Y, ldy * cw, B * cw, neg_lam, cw);
+  KERNEL_CHECK(c, "k_mass_sf");
+  return pawfe_apply_nonlocal<TX, TD, TD>(c, OpData<TD>::dS(c), -1.0, X, ldx, 0, Y, ldy, 0, B, lam);
+}
+template pawfe_status pawfe_sub_SX_lambda<float, double>(pawfe_ctx*, const float*, long, double*, long, int, const double*, const double*);
+template pawfe_status pawfe_sub_SX_lambda<double, double>(pawfe_ctx*, const double*, long, double*, long, int, const double*, const double*);
+template pawfe_status pawfe_sub_SX_lambda<float2, double2>(pawfe_ctx*, const float2*, long, double2*, long, int, const double*, const double*);
+template pawfe_status pawfe_sub_SX_lambda<double2, double2>(pawfe_ctx*, const double2*, long, double2*, long, int, const double*, const double*);
 
 // explicit instantiations used by the other translation units
 #define INST(TX, TY, TC)                                                                                          \
@@ -282,7 +311,7 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
       pawfe_status st = tc_cell_apply(c, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, 2 * B, 1.0f);
       prof_end(c);
       TRY(st);
-      return pawfe_apply_nonlocal<float2, float2, float2>(c, OpData<float2>::D(c), 1.0, (const float2*)X, ldx, 0, (float2*)Y, ldy, 0, B);
+      return pawfe_apply_nonlocal<float2, float2, float2>(c, OpData<float2>::D(c), 1.0, (const float2*)X, ldx, 0, (float2*)Y, ldy, 0, B, nullptr);
     }
     return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
   }
@@ -294,7 +323,7 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
     pawfe_status st = tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f);
     prof_end(c);
     TRY(st);
-    return pawfe_apply_nonlocal<float, float, float>(c, OpData<float>::D(c), 1.0, (const float*)X, ldx, 0, (float*)Y, ldy, 0, B);
+    return pawfe_apply_nonlocal<float, float, float>(c, OpData<float>::D(c), 1.0, (const float*)X, ldx, 0, (float*)Y, ldy, 0, B, nullptr);
   }
   return pawfe_apply_HS<float, float, float>(c, 0, tf32, (const float*)X, ldx, (float*)Y, ldy, B);
 }

@@ -9,6 +9,7 @@
 #include "fused.h"
 #include <algorithm>
 #include <cstring>
+#include <type_traits>
 
 namespace {
 
@@ -118,16 +119,26 @@ pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double
 
   // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
   TRY((pawfe_apply_HS<TS, TD, TD>(c, 0, false, X, ld, Y64, B, B)));
-  TRY((pawfe_apply_HS<TS, TD, TD>(c, 1, false, X, ld, SX64, B, B)));
+  (void)SX64;   // S X is not stored: Y -= (S X) Lambda directly (mass part by 1-D sweeps, Lambda folded into the coupling)
+  TRY((pawfe_sub_SX_lambda<TS, TD>(c, X, ld, Y64, B, B, ds, ds + (size_t)(m + 1) * B)));
   const int gs = 8 * c->sm_count;
   // ---- step 3 ----
-  k_residual_init<RS><<<gs, 256, 0, c->stream>>>(c->M, W, cw, (double*)Y64, (const double*)SX64, ds, z_over_e,
+  k_residual_init<RS><<<gs, 256, 0, c->stream>>>(c->M, W, cw, (double*)Y64, (const double*)nullptr, ds, z_over_e,
                                                  (RS*)RX, (RS*)RY);
   KERNEL_CHECK(c, "k_residual_init");
   // ---- step 4 ----
   for (int th = 2; th <= m; ++th) {
     TRY((pawfe_apply_Sinv_impl<TS, TS, TS>(c, RY, B, T, B, B)));
     TRY(pawfe_apply_H_any(c, prec, T, B, HT, B, B));
+    if constexpr (std::is_same<RS, float>::value) {
+      if ((W & 3) == 0) {
+        k_recurrence_f4<<<gs, 256, 0, c->stream>>>(total / 4, W / 4, cw, (const float4*)HT, (const float4*)RY, (float4*)RX,
+                                                   (const double2*)Y64, ds + (size_t)(th - 1) * B, (float)as[th], (float)acs[th], (float)zzs[th]);
+        KERNEL_CHECK(c, "k_recurrence_f4");
+        std::swap(RX, RY);
+        continue;
+      }
+    }
     k_recurrence<RS><<<gs, 256, 0, c->stream>>>(total, W, cw, (const RS*)HT, (const RS*)RY, (RS*)RX,
                                                 (const double*)Y64, ds + (size_t)(th - 1) * B, as[th], acs[th], zzs[th]);
     KERNEL_CHECK(c, "k_recurrence");

@@ -6,6 +6,10 @@
 template <typename TX, typename TY, typename TC>
 pawfe_status pawfe_apply_HS(pawfe_ctx* c, int op /*0 = H, 1 = S*/, bool tf32, const TX* X, long ldx, TY* Y,
                             long ldy, int B);
+// Y -= (S X) Lambda in FP64 without storing S X (api_apply.cu).
+template <typename TX, typename TD>
+pawfe_status pawfe_sub_SX_lambda(pawfe_ctx* c, const TX* X, long ldx, TD* Y, long ldy, int B, const double* lam,
+                                 const double* neg_lam);
 template <typename TX, typename TY, typename TC>
 pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, long ldy, int B);
 

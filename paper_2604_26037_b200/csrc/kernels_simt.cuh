@@ -142,9 +142,10 @@ k_proj(MeshDev md, int atom0, const int* __restrict__ aps, const int* __restrict
 }
 
 // W^a = scale * Delta^a P^a  (npj x npj times npj x B).  grid = (natoms, ceil(B/128)), block 128.
+// colscale (optional, device, [B] doubles): extra real factor per vector, e.g. the Ritz values Lambda.
 template <typename TC>
 __global__ void k_coupling(const TC* __restrict__ Delta, int npj, const TC* __restrict__ P, int ldp,
-                           int B, double scale, TC* __restrict__ W) {
+                           int B, double scale, TC* __restrict__ W, const double* __restrict__ colscale = nullptr) {
   const int a = blockIdx.x;
   const int v = blockIdx.y * blockDim.x + threadIdx.x;
   if (v >= B) return;
@@ -157,7 +158,7 @@ __global__ void k_coupling(const TC* __restrict__ Delta, int npj, const TC* __re
 #pragma unroll
     for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
       if (be < npj) s_fma(s, Delta[((long)a * npj + al) * npj + be], p[be]);
-    W[((long)a * npj + al) * ldp + v] = s_scale(s, scale);
+    W[((long)a * npj + al) * ldp + v] = s_scale(s, colscale ? scale * colscale[v] : scale);
   }
 }
 

@@ -48,7 +48,7 @@ __global__ void k_residual_init(long M, int W, int cw, double* __restrict__ HX,
   for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total;
        idx += (long)gridDim.x * blockDim.x) {
     int c = (int)(idx % W);
-    double y = HX[idx] - SX[idx] * lam[c / cw];
+    double y = SX ? HX[idx] - SX[idx] * lam[c / cw] : HX[idx];
     HX[idx] = y;
     RY[idx] = (TS)(z_over_e * y);
     RX[idx] = (TS)0;
@@ -112,4 +112,38 @@ __global__ void k_col_sumsq(long M, int B, int cw, const TS* __restrict__ X, lon
 static __global__ void k_sqrt_inplace(double* x, int n) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) x[i] = sqrt(x[i]);
+}
+
+// ---- float4-vectorised variants for FP32 storage (W % 4 == 0, 16-byte aligned rows); one row factor per thread row ----
+// Y = M_D^-1 X, 4 consecutive columns per thread.  Wq = W / 4; ldxq, ldyq = leading dimensions / 4.
+static __global__ void __launch_bounds__(256)
+k_scale_mdinv_f4(MeshDev md, const float4* __restrict__ X, long ldxq, float4* __restrict__ Y, long ldyq, int Wq) {
+  const long total = md.M * (long)Wq;
+  for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x) {
+    const long J = q / Wq;
+    const int c = (int)(q - J * Wq);
+    const float s = (float)mdinv_of_row(md, J);
+    const float4 x = X[J * ldxq + c];
+    Y[J * ldyq + c] = make_float4(x.x * s, x.y * s, x.z * s, x.w * s);
+  }
+}
+
+// Alg. 2 step 4 (L272) for FP32 storage, 4 consecutive real columns per thread (all blocks have leading dimension W):
+//   R_X <- a HT - a c R_Y - zeta zeta1 R_X  [FP32]  + a Y LamY [FP64 add]
+static __global__ void __launch_bounds__(256)
+k_recurrence_f4(long nquads, int Wq, int cw, const float4* __restrict__ HT, const float4* __restrict__ RY,
+                float4* __restrict__ RX, const double2* __restrict__ Y, const double* __restrict__ aLamY, float a,
+                float ac, float zz1) {
+  for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < nquads; q += (long)gridDim.x * blockDim.x) {
+    const int c0 = (int)(q % Wq) * 4;
+    const float4 h = HT[q], ry = RY[q], rx = RX[q];
+    const double2 y0 = Y[2 * q], y1 = Y[2 * q + 1];
+    const double l0 = aLamY[c0 / cw], l1 = aLamY[(c0 + 1) / cw], l2 = aLamY[(c0 + 2) / cw], l3 = aLamY[(c0 + 3) / cw];
+    float4 o;
+    o.x = (float)((double)(a * h.x - ac * ry.x - zz1 * rx.x) + y0.x * l0);
+    o.y = (float)((double)(a * h.y - ac * ry.y - zz1 * rx.y) + y0.y * l1);
+    o.z = (float)((double)(a * h.z - ac * ry.z - zz1 * rx.z) + y1.x * l2);
+    o.w = (float)((double)(a * h.w - ac * ry.w - zz1 * rx.w) + y1.y * l3);
+    RX[q] = o;
+  }
 }

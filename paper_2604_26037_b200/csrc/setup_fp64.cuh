@@ -8,12 +8,12 @@
 #pragma once
 #include "common.h"
 
-// Y[J][v] += coef[v] * (M^e X_e)[I][v] over all cells (coef = null: +1).  grid = (ncell, ceil(W/32)), block = 256.
+// Y[J][v] += coef[v / cw] * (M^e X_e)[I][v] over all cells (coef = null: +1; cw = 2: interleaved complex columns).  grid = (ncell, ceil(W/32)), block = 256.
 //   dynamic smem: n * 32 doubles + n longs.  M1: [n1][n1] doubles (device).
 template <typename RX>
 __global__ void __launch_bounds__(256)
 k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __restrict__ X, long ldx,
-          double* __restrict__ Y, long ldy, int W, const double* __restrict__ coef) {
+          double* __restrict__ Y, long ldy, int W, const double* __restrict__ coef, int cw = 1) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = md.n, n1 = md.n1, n2 = n1 * n1;
   double* U = reinterpret_cast<double*>(smem_raw);    // [n][32]
@@ -63,7 +63,7 @@ k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __r
   for (int i = threadIdx.x; i < n * 32; i += blockDim.x) {
     const int I = i >> 5, col = i & 31;
     const long J = nodeJ[I];
-    if (J >= 0 && v0 + col < W) atomicAdd(Y + J * ldy + v0 + col, (coef ? coef[v0 + col] : 1.0) * scale * U[i]);
+    if (J >= 0 && v0 + col < W) atomicAdd(Y + J * ldy + v0 + col, (coef ? coef[(v0 + col) / cw] : 1.0) * scale * U[i]);
   }
 }
 
