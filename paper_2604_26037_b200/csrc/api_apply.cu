@@ -315,8 +315,8 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
     }
     return pawfe_apply_HS<float2, float2, float2>(c, 0, tf32, (const float2*)X, ldx, (float2*)Y, ldy, B);
   }
-  if (tf32 && tc_usable(c, X, ldx, Y, ldy, B) && fused_supported(c, prec, B))
-    return fused_apply_H(c, (const float*)X, ldx, (float*)Y, ldy, B);
+  if (tc_usable(c, X, ldx, Y, ldy, B) && fused_supported(c, prec, B))
+    return fused_apply_H(c, prec, (const float*)X, ldx, (float*)Y, ldy, B);
   if (tf32 && tc_usable(c, X, ldx, Y, ldy, B)) {
     TRY(zero_block(c, (float*)Y, ldy, B));
     prof_begin(c);
@@ -331,7 +331,7 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
 extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec prec, int B) {
   if (!c) return "none";
   if (prec == PAWFE_FP64) return "dmma_fp64";
-  if (prec == PAWFE_FP32) return "simt_fp32";
+  if (prec == PAWFE_FP32) return (!c->cplx && tc_supported(c, B)) ? "tcgen05_3xtf32" : "simt_fp32";
   if (tc_supported(c, B)) return "tcgen05_tf32";
   return "simt_tf32_emulated";
 }

@@ -173,7 +173,7 @@ extern "C" pawfe_status pawfe_filter_workspace(pawfe_ctx* c, pawfe_prec prec, in
   if (fused_supported(c, prec, B)) {
     // fused step (fused.h): Yt (FP64) + Rt_X + Rt_Y (FP32); S X, T and H T are never stored
     const size_t ldw = ((size_t)B + 3) / 4 * 4;
-    *bytes = align256((size_t)c->M * ldw * 8) + 2 * align256((size_t)c->M * ldw * 4);
+    *bytes = align256((size_t)c->M * ldw * 8) + (prec == PAWFE_FP32 ? 3 : 2) * align256((size_t)c->M * ldw * 4);
   }
   return PAWFE_OK;
 }
@@ -194,7 +194,7 @@ extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, 
   if (fused_supported(c, prec, B)) {
     FilterScalars fs;
     TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
-    return fused_filter_real(c, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, (float*)X, ld, B, workspace);
+    return fused_filter_real(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, (float*)X, ld, B, workspace);
   }
   return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace);
 }

@@ -25,6 +25,9 @@ struct FusedPlan {
   int Bcap = 0; long ldw = 0;
   float* d_P1 = nullptr;        // [natoms][npj][ldw]
   float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
+  float* d_Wcat_lo = nullptr;   // low parts of Wcat (FP32 mode, 3xTF32 split)
+  float* d_Bext_lo = nullptr;   // low parts of d_Bext (built on first FP32-mode use)
+  float* d_xlo = nullptr; size_t xlo_elems = 0;   // low parts of the input block of fused_apply_H in FP32 mode
   double* d_P64 = nullptr;      // [natoms][npj][ldw] FP64 projections of the residual set-up
   double* d_W64 = nullptr;      // [natoms][npj][ldw] (D - Lambda dS) P
 };
@@ -389,6 +392,7 @@ void free_plan(FusedPlan* p) {
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
   cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD);
   cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
+  cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
   delete p;
 }
 
@@ -501,12 +505,14 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
 pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int B) {
   if (B <= p->Bcap) return PAWFE_OK;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
+  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64); cudaFree(p->d_Wcat_lo);
+  p->d_Wcat_lo = nullptr;
   p->d_P1 = p->d_Wcat = nullptr; p->d_P64 = p->d_W64 = nullptr; p->Bcap = 0;
   const long ldw = roundup4(B);
   const size_t na = (size_t)std::max(1, c->natoms);
   TRY(dev_alloc(c, &p->d_P1, na * c->npj * ldw));
   TRY(dev_alloc(c, &p->d_Wcat, na * 32 * ldw));
+  TRY(dev_alloc(c, &p->d_Wcat_lo, na * 32 * ldw));
   TRY(dev_alloc(c, &p->d_P64, na * c->npj * ldw));
   TRY(dev_alloc(c, &p->d_W64, na * c->npj * ldw));
   CUDA_TRY(c, cudaMemsetAsync(p->d_Wcat, 0, na * 32 * ldw * sizeof(float), c->stream));
@@ -594,7 +600,7 @@ void fused_invalidate(pawfe_ctx* c) {
 }
 
 bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
-  return prec == PAWFE_TF32 && !c->cplx && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
+  return (prec == PAWFE_TF32 || prec == PAWFE_FP32) && !c->cplx && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
 }
 
 pawfe_status fused_prepare(pawfe_ctx* c, int B) {
@@ -608,20 +614,57 @@ pawfe_status fused_prepare(pawfe_ctx* c, int B) {
   return ensure_scratch(c, p, B);
 }
 
-pawfe_status fused_apply_H(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B) {
-  TRY(fused_prepare(c, B));
-  FusedPlan* p = (FusedPlan*)c->fused;
-  TRY(project_and_couple(c, p, X, ldx, B, 2));
-  if (ldy == B) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * B * sizeof(float), c->stream));
-  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)B * sizeof(float), c->M, c->stream));
-  TcExt x = make_ext(p, 0);
+// One cell-level pass  Y += alpha [M_D^-1] (H_loc X + K-extension terms).  TF32: one launch.  FP32 ("FP32"):
+// three launches with the operands split into the part the tensor core keeps (hi = trunc_tf32) and the rest (lo):
+//   hi x hi + lo x hi + hi x lo   (the dropped lo x lo term is ~2^-22 relative), FP32 accumulation throughout.
+// xlo: scratch for the low parts of X (same shape).  Wcat holds the couplings of this step.
+pawfe_status cell_pass(pawfe_ctx* c, FusedPlan* p, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B,
+                       float alpha, int scale_mode, float* xlo) {
+  TcExt x = make_ext(p, scale_mode);
+  x.Hstream = nullptr;
   prof_begin(c);
-  pawfe_status st = tc_cell_apply(c, X, ldx, Y, ldy, B, 1.0f, &x);
+  pawfe_status st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x);
+  if (st == PAWFE_OK && prec == PAWFE_FP32) {
+    const float* hlo = nullptr;
+    st = tc_hstream_lo(c, &hlo);
+    if (st == PAWFE_OK && p->nchunks > 0 && !p->d_Bext_lo) {
+      int NH = 1, NT = c->n;
+      tc_shape(c, &NH, &NT);
+      const size_t cnt = (size_t)p->nchunks * NH * NT * 32;
+      st = dev_alloc(c, &p->d_Bext_lo, cnt);
+      if (st == PAWFE_OK) st = tc_lo_part(c, p->d_Bext, p->d_Bext_lo, (long)cnt);
+    }
+    if (st == PAWFE_OK) st = tc_lo_part(c, X, xlo, c->M * ldx);
+    if (st == PAWFE_OK && c->natoms > 0) st = tc_lo_part(c, p->d_Wcat, p->d_Wcat_lo, (long)c->natoms * 32 * p->ldw);
+    if (st == PAWFE_OK) {           // lo(X) x hi(H)
+      TcExt x2 = x; x2.Wcat = p->d_Wcat_lo;
+      st = tc_cell_apply(c, xlo, ldx, Y, ldy, B, alpha, &x2);
+    }
+    if (st == PAWFE_OK) {           // hi(X) x lo(H)
+      TcExt x3 = x; x3.Bext = p->d_Bext_lo; x3.Hstream = hlo;
+      st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x3);
+    }
+  }
   prof_end(c);
   return st;
 }
 
-pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const double* as, const double* acs,
+pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B) {
+  TRY(fused_prepare(c, B));
+  FusedPlan* p = (FusedPlan*)c->fused;
+  if (prec == PAWFE_FP32 && p->xlo_elems < (size_t)c->M * ldx) {
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(p->d_xlo); p->d_xlo = nullptr; p->xlo_elems = 0;
+    TRY(dev_alloc(c, &p->d_xlo, (size_t)c->M * ldx));
+    p->xlo_elems = (size_t)c->M * ldx;
+  }
+  TRY(project_and_couple(c, p, X, ldx, B, 2));
+  if (ldy == B) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * B * sizeof(float), c->stream));
+  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)B * sizeof(float), c->M, c->stream));
+  return cell_pass(c, p, prec, X, ldx, Y, ldy, B, 1.0f, 0, p->d_xlo);
+}
+
+pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds, const double* as, const double* acs,
                                const double* zzs, double z_over_e, float* X, long ld, int B, void* workspace) {
   TRY(fused_prepare(c, B));
   FusedPlan* p = (FusedPlan*)c->fused;
@@ -632,6 +675,7 @@ pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const doub
   double* Yt = (double*)ws;
   float* RX = (float*)(ws + blk_d);
   float* RY = (float*)(ws + blk_d + blk_s);
+  float* XLO = (float*)(ws + blk_d + 2 * blk_s);   // FP32 mode only (pawfe_filter_workspace adds the block)
   // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda, fused (setup_fp64.cuh): S X is never stored ----
   CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
   TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
@@ -648,17 +692,13 @@ pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds, const doub
   k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
-  TcExt x = make_ext(p, 1);
   const long nquads = c->M * (ldw / 4);
   for (int th = 2; th <= m; ++th) {
     TRY(project_and_couple(c, p, RY, ldw, B, 0));
     k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
                                          ds + (size_t)(th - 1) * B, B, (float)acs[th], (float)zzs[th]);
     KERNEL_CHECK(c, "k_prepass");
-    prof_begin(c);
-    pawfe_status st = tc_cell_apply(c, RY, ldw, RX, ldw, B, (float)as[th], &x);
-    prof_end(c);
-    TRY(st);
+    TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, B, (float)as[th], 1, XLO));
     std::swap(RX, RY);
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----

@@ -50,6 +50,8 @@ struct TcArgs {
 };
 
 struct TcPlan {
+  float* d_H32t_lo = nullptr;    // low parts (value - trunc_tf32(value)) of d_H32t, FP32 mode only
+  long h32t_elems = 0;
   float* d_H32t = nullptr;       // cell matrices re-tiled for streaming: [cell][half][K chunk][NT rows][32] floats
   int NT = 0, NH = 0;
   bool ok = false;
@@ -362,6 +364,7 @@ TcPlan* get_plan(pawfe_ctx* c) {
   const int kchunks = (c->ldk + kChunkK - 1) / kChunkK;
   const long elems = (long)c->ncell * p->NH * kchunks * ncomp * p->NT * 32;
   if (cudaMalloc((void**)&p->d_H32t, (size_t)elems * sizeof(float)) != cudaSuccess) { cudaGetLastError(); p->d_H32t = nullptr; return p; }
+  p->h32t_elems = elems;
   k_retile_h32<<<8 * c->sm_count, 256, 0, c->stream>>>((const float*)c->d_H32, c->n, c->ldk, p->NH, p->NT, kchunks, ncomp, elems, p->d_H32t);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) return p;
@@ -383,8 +386,37 @@ TcPlan* get_plan(pawfe_ctx* c) {
 
 void tc_shape(const pawfe_ctx* c, int* NH, int* NT) { shape_for(c, NH, NT); }
 
+namespace {
+__global__ void k_lo_part(const float* __restrict__ src, float* __restrict__ dst, long count) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < count; i += (long)gridDim.x * blockDim.x) {
+    const float v = src[i];
+    dst[i] = v - __uint_as_float(__float_as_uint(v) & 0xffffe000u);   // kind::tf32 keeps sign, exponent, 10 mantissa bits
+  }
+}
+}  // namespace
+
+pawfe_status tc_lo_part(pawfe_ctx* c, const float* src, float* dst, long count) {
+  k_lo_part<<<8 * c->sm_count, 256, 0, c->stream>>>(src, dst, count);
+  KERNEL_CHECK(c, "k_lo_part");
+  return PAWFE_OK;
+}
+
+pawfe_status tc_hstream_lo(pawfe_ctx* c, const float** out) {
+  TcPlan* p = get_plan(c);
+  if (!p->ok) { c->err = "tcgen05 cell kernel: plan set-up failed"; return PAWFE_EUNSUPPORTED; }
+  if (!p->d_H32t_lo) {
+    if (cudaMalloc((void**)&p->d_H32t_lo, (size_t)p->h32t_elems * sizeof(float)) != cudaSuccess) {
+      cudaGetLastError(); p->d_H32t_lo = nullptr; c->err = "out of memory for the low parts of the cell matrices"; return PAWFE_ENOMEM;
+    }
+    pawfe_status st = tc_lo_part(c, p->d_H32t, p->d_H32t_lo, p->h32t_elems);
+    if (st != PAWFE_OK) return st;
+  }
+  *out = p->d_H32t_lo;
+  return PAWFE_OK;
+}
+
 void tc_invalidate(pawfe_ctx* c) {
-  if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
+  if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t_lo); cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
 }
 
 bool tc_supported(const pawfe_ctx* c, int B) {
@@ -419,7 +451,7 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.tmem_cols = 2 * cols;
   a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
   a.scale_mode = 0;
-  a.H32t = p->d_H32t; a.Bext = nullptr;
+  a.H32t = (ext && ext->Hstream) ? ext->Hstream : p->d_H32t; a.Bext = nullptr;
   a.ext_start = nullptr; a.ext_atom = nullptr; a.Wcat = nullptr; a.ldw = 0; a.ext_ksteps = 0;
   if (ext) {
     a.scale_mode = ext->scale_mode;

@@ -27,7 +27,13 @@ struct TcExt {
   const float* Bext;           // [chunk][half][NT][32] floats, rows 128-byte swizzled (api_fused.cu k_build_ext)
   const float* Wcat; long ldw;
   int ksteps;
+  const float* Hstream;        // null: the context's re-tiled cell matrices; else an array of the same layout (tc_hstream_lo)
 };
+
+// dst[i] = src[i] - trunc_tf32(src[i]): the part of an FP32 value the tensor core drops (3xTF32 split, FP32 mode).
+pawfe_status tc_lo_part(pawfe_ctx* ctx, const float* src, float* dst, long count);
+// The low parts of the re-tiled cell-matrix stream (built on first use; same layout as the stream itself).
+pawfe_status tc_hstream_lo(pawfe_ctx* ctx, const float** out);
 
 // Y += alpha * [M_D^-1] sum_e P_e^T (H^e (P_e X) + extension terms) for a real FP32 block, TF32 multiply, FP32
 // accumulate.  X, Y: device [dof][vec] float, leading dimensions ldx, ldy.  Y must already hold the values to

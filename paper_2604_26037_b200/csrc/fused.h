@@ -23,11 +23,12 @@ void fused_invalidate(pawfe_ctx* c);
 // The couplings D changed: nothing to rebuild (D is read at run time), kept for symmetry.
 bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B);
 
-// Algorithm 2 for a real context in FP32 storage with the TF32 tcgen05 contraction.  Coefficients come from
+// Algorithm 2 for a real context in FP32 storage with the tcgen05 contraction: PAWFE_TF32 (one TF32 pass) or PAWFE_FP32
+// (three passes on hi/lo operand splits, FP32-accurate).  Coefficients come from
 // pawfe_filter_scalars (api_filter.cu).  X: [dof][vec] float, ld >= B.  workspace as pawfe_filter_workspace.
-pawfe_status fused_filter_real(pawfe_ctx* c, int m, const double* ds /*device scalars*/, const double* as,
+pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds /*device scalars*/, const double* as,
                                const double* acs, const double* zzs, double z_over_e, float* X, long ld, int B,
                                void* workspace);
 
 // Y = H X (TF32 contraction, non-local term through the K-extension).  X, Y float, 16-byte aligned, ld % 4 == 0.
-pawfe_status fused_apply_H(pawfe_ctx* c, const float* X, long ldx, float* Y, long ldy, int B);
+pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B);

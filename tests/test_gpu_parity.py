@@ -186,13 +186,13 @@ def test_full_size_cfg1_H_sampled_rows():
     """H X at 884,736 dofs x 200 vectors (tcgen05 kernel, two vector tiles, K-extension) against the oracle's
     row-by-row evaluation (oracle.operators.apply_H_rows) on the nodes of two sampled cells."""
     from oracle.operators import apply_H_rows
-    from paper_2604_26037_b200 import TF32, FP64
+    from paper_2604_26037_b200 import TF32, FP32, FP64
     cfg, sysd, ctx = _full_cfg1()
     B = cfg.block
     X = random_block(cfg, B, stream=11)
     cells = [(0, 0, 0), (7, 15, 3)]          # a corner cell (periodic wrap) and an interior one
     want = apply_H_rows(sysd, X, cells)
-    for prec, name, tol in ((TF32, "tf32", TOL["tf32"]), (FP64, "fp64", TOL["fp64"])):
+    for prec, name, tol in ((TF32, "tf32", TOL["tf32"]), (FP32, "fp32", TOL["fp32"]), (FP64, "fp64", TOL["fp64"])):
         Xd = _to_dev(X, name, False)
         Yd = torch.empty_like(Xd)
         ctx.apply_H(prec, Xd, Yd, B, B)
