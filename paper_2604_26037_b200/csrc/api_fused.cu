@@ -28,6 +28,8 @@ struct FusedPlan {
   float* d_Wcat_lo = nullptr;   // low parts of Wcat (FP32 mode, 3xTF32 split)
   float* d_Bext_lo = nullptr;   // low parts of d_Bext (built on first FP32-mode use)
   float* d_xlo = nullptr; size_t xlo_elems = 0;   // low parts of the input block of fused_apply_H in FP32 mode
+  // second stream for work that is independent inside a step (projection || bracket prepass; mass / non-local || DMMA)
+  cudaStream_t aux = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   double* d_P64 = nullptr;      // [natoms][npj][ldw] FP64 projections of the residual set-up
   double* d_W64 = nullptr;      // [natoms][npj][ldw] (D - Lambda dS) P
 };
@@ -393,6 +395,9 @@ void free_plan(FusedPlan* p) {
   cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD);
   cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
   cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
+  if (p->aux) cudaStreamDestroy(p->aux);
+  if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+  if (p->ev_join) cudaEventDestroy(p->ev_join);
   delete p;
 }
 
@@ -603,11 +608,25 @@ bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
   return (prec == PAWFE_TF32 || prec == PAWFE_FP32) && !c->cplx && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
 }
 
+// run `body` on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream
+#define FORK_AUX(c, p) do { CUDA_TRY(c, cudaEventRecord((p)->ev_fork, (c)->stream)); CUDA_TRY(c, cudaStreamWaitEvent((p)->aux, (p)->ev_fork, 0)); } while (0)
+#define JOIN_AUX(c, p) do { CUDA_TRY(c, cudaEventRecord((p)->ev_join, (p)->aux)); CUDA_TRY(c, cudaStreamWaitEvent((c)->stream, (p)->ev_join, 0)); } while (0)
+struct StreamSwap {   // kernels launched while this lives go to `s`
+  pawfe_ctx* c; cudaStream_t keep;
+  StreamSwap(pawfe_ctx* c_, cudaStream_t s) : c(c_), keep(c_->stream) { c->stream = s; }
+  ~StreamSwap() { c->stream = keep; }
+};
+
 pawfe_status fused_prepare(pawfe_ctx* c, int B) {
   FusedPlan* p = (FusedPlan*)c->fused;
   if (!p) {
     p = new FusedPlan();
     c->fused = p;
+    if (cudaStreamCreateWithFlags(&p->aux, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError(); fused_invalidate(c); c->err = "fused plan: stream / event creation failed"; return PAWFE_ECUDA;
+    }
     pawfe_status st = build_plan(c, p);
     if (st != PAWFE_OK) { fused_invalidate(c); return st; }
   }
@@ -678,26 +697,31 @@ pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const doubl
   float* XLO = (float*)(ws + blk_d + 2 * blk_s);   // FP32 mode only (pawfe_filter_workspace adds the block)
   // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda, fused (setup_fp64.cuh): S X is never stored ----
   CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
-  TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
+  FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
+  TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
   {
+    StreamSwap sw(c, p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
     const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
     static size_t smem_attr = 0;
     if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_mass_sf<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
     k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
         c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
     KERNEL_CHECK(c, "k_mass_sf");
+    if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
   }
+  JOIN_AUX(c, p);
   const int gs = 8 * c->sm_count;
-  if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
   k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
   const long nquads = c->M * (ldw / 4);
   for (int th = 2; th <= m; ++th) {
-    TRY(project_and_couple(c, p, RY, ldw, B, 0));
+    FORK_AUX(c, p);
+    { StreamSwap sw(c, p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
     k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
                                          ds + (size_t)(th - 1) * B, B, (float)acs[th], (float)zzs[th]);
     KERNEL_CHECK(c, "k_prepass");
+    JOIN_AUX(c, p);
     TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, B, (float)as[th], 1, XLO));
     std::swap(RX, RY);
   }
