@@ -145,6 +145,25 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+# multi-rank host logic (replicas only: no collective on the data path)
+# ------------------------------------------------------------------------------------------------
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """Slowest rank's time: the job's time (bench contract).  Works with nccl (device tensor) and gloo (CPU)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_per_step: float, steps: int, world: int, ms_max: float) -> float:
+    """Aggregate throughput of `world` replicas that each processed the same units in ms_max (max over ranks)."""
+    return world * units_per_rank_per_step * steps / (ms_max * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
 # own arm
 # ------------------------------------------------------------------------------------------------
 def run_own(args):
@@ -242,10 +261,7 @@ def run_own(args):
     ctx.cell_timing(False)
     launches = ctx.launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     finite = all(bool(torch.isfinite(x).all()) for blks in ring for x in blks) and (scratch is None or bool(torch.isfinite(scratch).all()))
 
     # end to end through the C ABI with HOST buffers: H2D of each block, filter, D2H of Psi_f, inside the timed region
@@ -267,17 +283,14 @@ def run_own(args):
         one(1 + k)
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     units = float(M) * N * m                      # per rank per step
-    value = world * units * args.steps / (ms * 1e-3)
+    value = whole_job_value(units, args.steps, world, ms)
     peaks = _peaks()
     n = (cfg.p + 1) ** 3
     ncell = cfg.ncells[0] * cfg.ncells[1] * cfg.ncells[2]
