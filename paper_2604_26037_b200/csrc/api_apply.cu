@@ -67,11 +67,7 @@ pawfe_status launch_dmma_mt(pawfe_ctx* c, const double* A, long cell_stride, con
                             int Wr, double alpha) {
   auto kern = dmma::k_cell_dmma<RX, CPLX, MT>;
   const size_t smem = dmma::smem_bytes<RX, CPLX, MT>(c->n);
-  static size_t smem_attr = 0;
-  if (smem > smem_attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    smem_attr = smem;
-  }
+  TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
   kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   KERNEL_CHECK(c, "k_cell_dmma");
   return PAWFE_OK;
@@ -101,11 +97,7 @@ pawfe_status launch_cell(pawfe_ctx* c, const TC* A, long cell_stride, int lda, c
   constexpr int BV = (sizeof(TC) == 16) ? 16 : 32;
   size_t smem = (size_t)c->n * 16 + (size_t)c->n * BV * sizeof(TC);
   auto kern = k_cell_simt<TX, TY, TC, BV, TF32>;
-  static size_t smem_attr = 0;  // per instantiation; the attribute is per function, so only ever raise it
-  if (smem > smem_attr) {
-    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    smem_attr = smem;
-  }
+  TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
   kern<<<dim3(c->ncell, ceil_div(B, BV)), 256, smem, c->stream>>>(c->md, A, cell_stride, lda, X, ldx, Y, ldy, B,
                                                                   in_scale, alpha);
   KERNEL_CHECK(c, "k_cell_simt");
@@ -127,8 +119,7 @@ pawfe_status nonlocal_f32_t(pawfe_ctx* c, const float* Delta, double scale, cons
   const size_t head = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16;
   {
     const size_t smem = head + ((size_t)NPJ * n * cw + 3) / 4 * 16 + (size_t)NPJ * 128 * 4;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_projF<NPJ, CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    TRY(pawfe_ensure_smem(c, (const void*)k_projF<NPJ, CPLX>, smem));
     k_projF<NPJ, CPLX><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx * cw, Wr,
                                                       in_scale, P, (long)Wr);
     KERNEL_CHECK(c, "k_projF");
@@ -137,10 +128,9 @@ pawfe_status nonlocal_f32_t(pawfe_ctx* c, const float* Delta, double scale, cons
   KERNEL_CHECK(c, "k_coupling");
   {
     const size_t smem = head + ((size_t)NPJ * n * cw + 3) / 4 * 16;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatterF<NPJ, CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
-    k_scatterF<NPJ, CPLX><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, W, (long)Wr, Wr,
-                                                         out_scale, Y, ldy * cw);
+    TRY(pawfe_ensure_smem(c, (const void*)k_scatterF<NPJ, CPLX>, smem));
+    k_scatterF<NPJ, CPLX><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, W, (long)Wr, NPJ, Wr,
+                                                         out_scale, 1.0f, Y, ldy * cw);
     KERNEL_CHECK(c, "k_scatterF");
   }
   return PAWFE_OK;
@@ -237,8 +227,7 @@ pawfe_status pawfe_sub_SX_lambda(pawfe_ctx* c, const TX* X, long ldx, TD* Y, lon
   typedef typename ScalarTraits<TX>::real RX;
   constexpr int cw = ScalarTraits<TX>::cplx ? 2 : 1;
   const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
-  static size_t smem_attr = 0;
-  if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_mass_sf<RX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+  TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<RX>, smem));
   k_mass_sf<RX><<<dim3(c->ncell, ceil_div(B * cw, 32)), 256, smem, c->stream>>>(
       c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, (const RX*)X, ldx * cw, (double*)Y, ldy * cw, B * cw, neg_lam, cw);
   KERNEL_CHECK(c, "k_mass_sf");
@@ -304,6 +293,8 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
   }
   bool tf32 = prec == PAWFE_TF32;
   if (c->cplx) {
+    if (tc_usable(c, X, 2 * ldx, Y, 2 * ldy, 2 * B) && fused_supported(c, prec, B))
+      return fused_apply_H(c, prec, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, B);
     if (tf32 && tc_usable(c, X, 2 * ldx, Y, 2 * ldy, 2 * B)) {
       // complex TF32: interleaved (re, im) columns as a real block of 2B columns; P / Q accumulators in the kernel
       TRY(zero_block(c, (float2*)Y, ldy, B));

@@ -162,19 +162,29 @@ pawfe_status check_filter(pawfe_ctx* c, pawfe_prec prec, int m, double b0, doubl
   return PAWFE_OK;
 }
 
+// bytes of workspace of the generic sequence (fused = false) or of the fused step
+size_t filter_ws_bytes(pawfe_ctx* c, pawfe_prec prec, int B, bool fused) {
+  size_t cw = c->cplx ? 2 : 1;
+  size_t ss = (prec == PAWFE_FP64 ? 8 : 4) * cw, sd = 8 * cw;
+  size_t bytes = ws_layout(c->M, B, ss, sd).total;
+  if (fused) {
+    // fused step (fused.h): Yt (FP64) + Rt_X + Rt_Y (FP32) as real blocks of B * cw columns; S X, T and H T are never
+    // stored.  Never more than the generic layout, so a block the fused path turns down (alignment) still fits.
+    const size_t ldw = ((size_t)B * cw + 3) / 4 * 4;
+    bytes = align256((size_t)c->M * ldw * 8) + (prec == PAWFE_FP32 ? 3 : 2) * align256((size_t)c->M * ldw * 4);
+  }
+  return bytes;
+}
+
+// complex blocks take the fused step only with an even width (16-byte pieces of interleaved columns)
+bool fused_width_ok(pawfe_ctx* c, pawfe_prec prec, int B) { return fused_supported(c, prec, B) && (!c->cplx || !(B & 1)); }
+
 }  // namespace
 
 extern "C" pawfe_status pawfe_filter_workspace(pawfe_ctx* c, pawfe_prec prec, int B, size_t* bytes) {
   if (!c || !bytes || B < 1 || B > 512) return PAWFE_EINVAL;
   if (!c->have_mesh) return PAWFE_ESTATE;
-  size_t cw = c->cplx ? 2 : 1;
-  size_t ss = (prec == PAWFE_FP64 ? 8 : 4) * cw, sd = 8 * cw;
-  *bytes = ws_layout(c->M, B, ss, sd).total;
-  if (fused_supported(c, prec, B)) {
-    // fused step (fused.h): Yt (FP64) + Rt_X + Rt_Y (FP32); S X, T and H T are never stored
-    const size_t ldw = ((size_t)B + 3) / 4 * 4;
-    *bytes = align256((size_t)c->M * ldw * 8) + (prec == PAWFE_FP32 ? 3 : 2) * align256((size_t)c->M * ldw * 4);
-  }
+  *bytes = filter_ws_bytes(c, prec, B, fused_width_ok(c, prec, B));
   return PAWFE_OK;
 }
 
@@ -182,19 +192,29 @@ extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, 
                                           void* X, const double* lambda, long ld, int B, void* workspace,
                                           size_t workspace_bytes) {
   TRY(check_filter(c, prec, m, b0, bW, bU, X, lambda, ld, B));
-  size_t need = 0;
-  TRY(pawfe_filter_workspace(c, prec, B, &need));
-  if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) { c->err = "workspace too small or misaligned"; return PAWFE_EINVAL; }
+  // complex blocks with an odd leading dimension or a misaligned pointer run the generic sequence (larger workspace)
+  const bool fused = fused_width_ok(c, prec, B) && (!c->cplx || (!(ld & 1) && !((uintptr_t)X & 15)));
+  const size_t need = filter_ws_bytes(c, prec, B, fused);
+  if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) {
+    c->err = fused ? "workspace too small or misaligned"
+                   : "workspace too small or misaligned (blocks the fused step cannot take need the generic sequence's workspace)";
+    return PAWFE_EINVAL;
+  }
   CUDA_TRY(c, cudaSetDevice(c->device));
   if (c->cplx) {
     if (prec == PAWFE_FP64) return filter_impl<double2, double2>(c, prec, m, b0, bW, bU, (double2*)X, lambda, ld, B, workspace);
+    if (fused) {
+      FilterScalars fs;
+      TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
+      return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace);
+    }
     return filter_impl<float2, double2>(c, prec, m, b0, bW, bU, (float2*)X, lambda, ld, B, workspace);
   }
   if (prec == PAWFE_FP64) return filter_impl<double, double>(c, prec, m, b0, bW, bU, (double*)X, lambda, ld, B, workspace);
-  if (fused_supported(c, prec, B)) {
+  if (fused) {
     FilterScalars fs;
     TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
-    return fused_filter_real(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, (float*)X, ld, B, workspace);
+    return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace);
   }
   return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace);
 }
@@ -204,8 +224,8 @@ extern "C" pawfe_status pawfe_cheb_filter_host(pawfe_ctx* c, pawfe_prec prec, in
   TRY(check_filter(c, prec, m, b0, bW, bU, X_host, lambda, ld, B));
   CUDA_TRY(c, cudaSetDevice(c->device));
   size_t es = (prec == PAWFE_FP64 ? 8 : 4) * (c->cplx ? 2 : 1);
-  size_t blk = (size_t)c->M * ld * es, need = 0;
-  TRY(pawfe_filter_workspace(c, prec, B, &need));
+  const size_t blk = (size_t)c->M * ld * es;
+  const size_t need = filter_ws_bytes(c, prec, B, fused_width_ok(c, prec, B) && (!c->cplx || !(ld & 1)));
   if (blk > c->hostblk_bytes) {
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     cudaFree(c->d_hostblk); c->d_hostblk = nullptr; c->hostblk_bytes = 0;

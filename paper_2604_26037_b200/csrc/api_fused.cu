@@ -7,6 +7,7 @@
 #include "api_internal.h"
 #include "apply_impl.h"
 #include "setup_fp64.cuh"
+#include "nonlocal_f32.cuh"
 #include <algorithm>
 #include <cmath>
 #include <set>
@@ -50,22 +51,37 @@ __device__ inline int find_pair(const int* __restrict__ aps, const int* __restri
 }
 
 // ------------------------------------------------------------------------------------------------
-// Set-up: one CTA per K-extension chunk x = (cell e, atom b).
-//   Zs[I][be] = M_D^-1[J] * (assembled C^b)[J][be] at the nodes J of cell e  (sum over the <= 8 cells sharing J)
-//   Bext[x][I][be]       = - sum_J H^e[I][J] Zs[J][be]                         (be < npj)
-//   Bext[x][I][npj + be] = C^{e,b}[I][be] if (e, b) is a pair, else 0
-//   G[slot(a, b)][al][be] += sum_I C^{e,a}[I][al] Zs[I][be]   for every pair (e, a)     (G^{ab} = C^a^T M_D^-1 C^b)
-// Real contexts only.  block = 256; dynamic smem: n * npj doubles.
+// Set-up: one CTA per K-extension chunk x = (cell e, atom b).  TD = double (real) or double2 (complex context).
+//   Zs[I][be] = M_D^-1[J] * (assembled C^b)[J][be] at the nodes J of cell e  (sum over the <= 8 cells sharing J);
+//               C^b = (C^b dagger)^dagger, i.e. conj of the stored rows Cd = C^{e,b dagger} (Eq. 34)
+//   block[I][be]       = - sum_J H^e[I][J] Zs[J][be]                         (be < npj)
+//   block[I][npj + be] = C^{e,b}[I][be] = conj(Cd[pair][be][I]) if (e, b) is a pair, else 0
+//   G[slot(a, b)][al][be] += sum_I Cd^{e,a}[al][I] Zs[I][be]   for every pair (e, a)   (G^{ab} = C^a^dagger M_D^-1 C^b)
+// Output layout [x][half][comp][NT rows][32] floats (comp: Re, Im), rows 128-byte swizzled (16-byte piece j of row r at
+// j ^ (r % 8)), the block format of the cell kernel; rows I >= n stay zero.  block = 256; smem: n * npj TD.
 // ------------------------------------------------------------------------------------------------
+__device__ inline double  t_conj(double a)  { return a; }
+__device__ inline double2 t_conj(double2 a) { return make_double2(a.x, -a.y); }
+__device__ inline double  t_re(double a)  { return a; }
+__device__ inline double  t_re(double2 a) { return a.x; }
+__device__ inline double  t_im(double)    { return 0.0; }
+__device__ inline double  t_im(double2 a) { return a.y; }
+__device__ inline void t_atomic_add(double* p, double v) { atomicAdd(p, v); }
+__device__ inline void t_atomic_add(double2* p, double2 v) { atomicAdd(&p->x, v.x); atomicAdd(&p->y, v.y); }
+__device__ inline double  t_warp_sum(double s)  { for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o); return s; }
+__device__ inline double2 t_warp_sum(double2 s) { return make_double2(t_warp_sum(s.x), t_warp_sum(s.y)); }
+
+template <typename TD>
 __global__ void __launch_bounds__(256)
 k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict__ ext_atom,
-            const int* __restrict__ aps, const int* __restrict__ pair_cell, const double* __restrict__ Cd64,
-            int npj, const double* __restrict__ H64, const int* __restrict__ cell_pair_start,
+            const int* __restrict__ aps, const int* __restrict__ pair_cell, const TD* __restrict__ Cd64,
+            int npj, const TD* __restrict__ H64, const int* __restrict__ cell_pair_start,
             const int* __restrict__ cell_pair_idx, const int* __restrict__ pair_atom,
             const int* __restrict__ nb_start, const int* __restrict__ nb_atom, int NH, int NT,
-            float* __restrict__ Bext, double* __restrict__ G) {
+            float* __restrict__ Bext, TD* __restrict__ G) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* Zs = reinterpret_cast<double*>(smem_raw);  // [n][npj]
+  constexpr int ncomp = ScalarTraits<TD>::cplx ? 2 : 1;
+  TD* Zs = reinterpret_cast<TD*>(smem_raw);  // [n][npj]
   const int n = md.n, n1 = md.n1, p = md.p;
   const int x = blockIdx.x;
   const int e = ext_cell[x], b = ext_atom[x];
@@ -89,7 +105,7 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
         if (nbc >= 0 && nbc < md.nc[d]) { ccell[d][1] = nbc; cloc[d][1] = nbl; ncand[d] = 2; }
       }
     }
-    for (int be = 0; be < npj; ++be) Zs[I * npj + be] = 0.0;
+    for (int be = 0; be < npj; ++be) Zs[I * npj + be] = s_zero(TD());
     if (mi != 0.0) {
       for (int qx = 0; qx < ncand[0]; ++qx)
         for (int qy = 0; qy < ncand[1]; ++qy)
@@ -98,43 +114,48 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
             const int pr = find_pair(aps, pair_cell, b, e2);
             if (pr < 0) continue;
             const int I2 = (cloc[0][qx] * n1 + cloc[1][qy]) * n1 + cloc[2][qz];
-            for (int be = 0; be < npj; ++be) Zs[I * npj + be] += Cd64[((long)pr * npj + be) * n + I2];
+            for (int be = 0; be < npj; ++be)
+              Zs[I * npj + be] = s_add(Zs[I * npj + be], t_conj(Cd64[((long)pr * npj + be) * n + I2]));
           }
-      for (int be = 0; be < npj; ++be) Zs[I * npj + be] *= mi;
+      for (int be = 0; be < npj; ++be) Zs[I * npj + be] = s_scale(Zs[I * npj + be], mi);
     }
   }
   __syncthreads();
   // ---- phase 2: K-extension block ----
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const int prb = find_pair(aps, pair_cell, b, e);
-  const double* He = H64 + (long)e * n * n;
-  // block layout of the cell kernel's operand stream: [x][half][NT rows][32], 128-byte swizzled per row
-  // (16-byte piece j of row r stored at j ^ (r % 8)); rows I >= n stay zero
-  auto bidx = [&](int I, int k) -> long {
+  const TD* He = H64 + (long)e * n * n;
+  auto bidx = [&](int I, int k, int comp) -> long {
     const int half = I / NT, r = I - half * NT;
-    return (((long)x * NH + half) * NT + r) * 32 + ((((k >> 2) ^ (r & 7)) << 2) | (k & 3));
+    return ((((long)x * NH + half) * ncomp + comp) * NT + r) * 32 + ((((k >> 2) ^ (r & 7)) << 2) | (k & 3));
   };
   for (int I = w; I < n; I += nw) {
-    double acc[PAWFE_MAX_NPJ];
+    TD acc[PAWFE_MAX_NPJ];
 #pragma unroll
-    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) acc[be] = 0.0;
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) acc[be] = s_zero(TD());
     for (int J = lane; J < n; J += 32) {
-      const double h = He[(long)I * n + J];
+      const TD h = He[(long)I * n + J];
 #pragma unroll
       for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
-        if (be < npj) acc[be] = fma(h, Zs[J * npj + be], acc[be]);
+        if (be < npj) s_fma(acc[be], h, Zs[J * npj + be]);
     }
 #pragma unroll
     for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
       if (be < npj) {
-        double s = acc[be];
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) Bext[bidx(I, be)] = (float)(-s);
+        const TD s = t_warp_sum(acc[be]);
+        if (lane == 0) {
+          Bext[bidx(I, be, 0)] = (float)(-t_re(s));
+          if (ncomp == 2) Bext[bidx(I, be, 1)] = (float)(-t_im(s));
+        }
       }
     for (int k = npj + lane; k < 32; k += 32) {
-      float v = 0.f;
-      if (k < 2 * npj && prb >= 0) v = (float)Cd64[((long)prb * npj + (k - npj)) * n + I];
-      Bext[bidx(I, k)] = v;
+      float vr = 0.f, vi = 0.f;
+      if (k < 2 * npj && prb >= 0) {
+        const TD cv = t_conj(Cd64[((long)prb * npj + (k - npj)) * n + I]);
+        vr = (float)t_re(cv); vi = (float)t_im(cv);
+      }
+      Bext[bidx(I, k, 0)] = vr;
+      if (ncomp == 2) Bext[bidx(I, k, 1)] = vi;
     }
   }
   // ---- phase 3: G^{ab} contributions of this cell ----
@@ -145,10 +166,10 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
     if (slot < 0) continue;
     for (int ab = w; ab < npj * npj; ab += nw) {
       const int al = ab / npj, be = ab % npj;
-      double s = 0.0;
-      for (int I = lane; I < n; I += 32) s = fma(Cd64[((long)pr * npj + al) * n + I], Zs[I * npj + be], s);
-      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-      if (lane == 0) atomicAdd(&G[((long)slot * npj + al) * npj + be], s);
+      TD s = s_zero(TD());
+      for (int I = lane; I < n; I += 32) s_fma(s, Cd64[((long)pr * npj + al) * n + I], Zs[I * npj + be]);
+      s = t_warp_sum(s);
+      if (lane == 0) t_atomic_add(&G[((long)slot * npj + al) * npj + be], s);
     }
   }
 }
@@ -229,51 +250,52 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
 //   mode 0: both (filter step);  mode 1: W only (recovery, S^-1approx alone);  mode 2: plain H (W = 0, W2 = D P1).
 //   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2.  grid = (natoms, ceil(B/128)), block = 128.
 // ------------------------------------------------------------------------------------------------
+template <typename T>   // float (real context) or float2 (complex context); ldp, ldw in units of T
 __global__ void __launch_bounds__(128)
-k_couple(int npj, int mode, const float* __restrict__ P1, long ldp, int B, const float* __restrict__ dSinv,
-         const float* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
-         const float* __restrict__ GD, float* __restrict__ Wcat, long ldw) {
+k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, const T* __restrict__ dSinv,
+         const T* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
+         const T* __restrict__ GD, T* __restrict__ Wcat, long ldw) {
   const int a = blockIdx.x;
   const int v = blockIdx.y * blockDim.x + threadIdx.x;
   if (v >= B) return;
-  float p1[PAWFE_MAX_NPJ], p2[PAWFE_MAX_NPJ];
+  T p1[PAWFE_MAX_NPJ], p2[PAWFE_MAX_NPJ];
 #pragma unroll
-  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) { p1[be] = be < npj ? P1[((long)a * npj + be) * ldp + v] : 0.f; p2[be] = p1[be]; }
-  float* Wa = Wcat + (long)a * 32 * ldw;
+  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) { p1[be] = be < npj ? P1[((long)a * npj + be) * ldp + v] : s_zero(T()); p2[be] = p1[be]; }
+  T* Wa = Wcat + (long)a * 32 * ldw;
   if (mode != 2) {
-    const float* S = dSinv + (long)a * npj * npj;
+    const T* S = dSinv + (long)a * npj * npj;
     for (int al = 0; al < npj; ++al) {
-      float s = 0.f;
+      T s = s_zero(T());
 #pragma unroll
-      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s = fmaf(S[al * npj + be], p1[be], s);
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[al * npj + be], p1[be]);
       Wa[(long)al * ldw + v] = s;
     }
   } else {
-    for (int al = 0; al < npj; ++al) Wa[(long)al * ldw + v] = 0.f;
+    for (int al = 0; al < npj; ++al) Wa[(long)al * ldw + v] = s_zero(T());
   }
   if (mode == 1) return;
   if (mode == 0) {
     for (int s = nb_start[a]; s < nb_start[a + 1]; ++s) {
       const int b = nb_atom[s];
-      const float* g = GD + (long)s * npj * npj;
-      float pb[PAWFE_MAX_NPJ];
+      const T* g = GD + (long)s * npj * npj;
+      T pb[PAWFE_MAX_NPJ];
 #pragma unroll
-      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) pb[be] = be < npj ? P1[((long)b * npj + be) * ldp + v] : 0.f;
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) pb[be] = be < npj ? P1[((long)b * npj + be) * ldp + v] : s_zero(T());
 #pragma unroll
       for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
         if (al < npj) {
-          float t = 0.f;
+          T t = s_zero(T());
 #pragma unroll
-          for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) t = fmaf(g[al * npj + be], pb[be], t);
-          p2[al] -= t;
+          for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(t, g[al * npj + be], pb[be]);
+          p2[al] = s_add(p2[al], s_scale(t, -1.0));
         }
     }
   }
-  const float* Da = D + (long)a * npj * npj;
+  const T* Da = D + (long)a * npj * npj;
   for (int al = 0; al < npj; ++al) {
-    float s = 0.f;
+    T s = s_zero(T());
 #pragma unroll
-    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s = fmaf(Da[al * npj + be], p2[be], s);
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, Da[al * npj + be], p2[be]);
     Wa[(long)(npj + al) * ldw + v] = s;
   }
 }
@@ -355,17 +377,17 @@ __global__ void k_residual_init2(MeshDev md, long ldw, int B, double* __restrict
 // 4 consecutive vectors per thread; ldw % 4 == 0.
 __global__ void __launch_bounds__(256)
 k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, float4* __restrict__ RX,
-          const double2* __restrict__ Yt, const double* __restrict__ aLamY, int B, float ac, float zz1) {
+          const double2* __restrict__ Yt, const double* __restrict__ aLamY, int B /*real columns*/, int cw, float ac, float zz1) {
   for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < nquads; q += (long)gridDim.x * blockDim.x) {
     const int v = (int)(q % ldq) * 4;
     const float4 ry = RY[q];
     const float4 rx = RX[q];
     const double2 y0 = Yt[2 * q], y1 = Yt[2 * q + 1];
     double l0 = 0, l1 = 0, l2 = 0, l3 = 0;
-    if (v < B) l0 = aLamY[v];
-    if (v + 1 < B) l1 = aLamY[v + 1];
-    if (v + 2 < B) l2 = aLamY[v + 2];
-    if (v + 3 < B) l3 = aLamY[v + 3];
+    if (v < B) l0 = aLamY[v / cw];
+    if (v + 1 < B) l1 = aLamY[(v + 1) / cw];
+    if (v + 2 < B) l2 = aLamY[(v + 2) / cw];
+    if (v + 3 < B) l3 = aLamY[(v + 3) / cw];
     float4 o;
     o.x = (float)((double)(-ac * ry.x - zz1 * rx.x) + y0.x * l0);
     o.y = (float)((double)(-ac * ry.y - zz1 * rx.y) + y0.y * l1);
@@ -377,15 +399,15 @@ k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, flo
 
 // Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
 // by k_scatter2.  keep = 0 on Dirichlet boundary rows.
-__global__ void k_recover2(MeshDev md, long ldw, int B, const float* __restrict__ RY, float* __restrict__ X, long ldx,
-                           const double* __restrict__ lamY) {
+__global__ void k_recover2(MeshDev md, long ldw, int B /*real columns*/, int cw, const float* __restrict__ RY, float* __restrict__ X,
+                           long ldx, const double* __restrict__ lamY) {
   const long total = md.M * (long)B;
   for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
     const long J = idx / B;
     const int v = (int)(idx - J * B);
     const double keep = mdinv_row(md, J) != 0.0 ? 1.0 : 0.0;
     const double x = (double)X[J * ldx + v];
-    X[J * ldx + v] = (float)(keep * ((double)RY[J * ldw + v] + x * lamY[v]));
+    X[J * ldx + v] = (float)(keep * ((double)RY[J * ldw + v] + x * lamY[v / cw]));
   }
 }
 
@@ -463,43 +485,57 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   TRYP(upload(c, &p->d_nb_start, ns)); TRYP(upload(c, &p->d_nb_atom, na));
   int NH = 1, NT = n;
   tc_shape(c, &NH, &NT);
-  TRYP(dev_alloc(c, &p->d_Bext, (size_t)p->nchunks * NH * NT * 32));
-  cudaMemsetAsync(p->d_Bext, 0, (size_t)p->nchunks * NH * NT * 32 * sizeof(float), c->stream);
-  TRYP(dev_alloc(c, &d_G, (size_t)nnb * npj * npj));
-  cudaMemsetAsync(d_G, 0, (size_t)nnb * npj * npj * sizeof(double), c->stream);
-  size_t smem = (size_t)n * npj * sizeof(double);
-  cudaError_t e = cudaFuncSetAttribute(k_build_ext, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) {
-    k_build_ext<<<(unsigned)p->nchunks, 256, smem, c->stream>>>(
-        c->md, d_ec, p->d_ext_atom, c->d_atom_pair_start, c->d_pair_cell, (const double*)c->d_Cd64, npj,
-        (const double*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, NH, NT, p->d_Bext, d_G);
-    c->launches++;
-    e = cudaGetLastError();
+  const int cw = c->cplx ? 2 : 1;
+  const size_t per2 = (size_t)npj * npj;
+  const size_t bext_elems = (size_t)p->nchunks * NH * NT * 32 * cw;
+  TRYP(dev_alloc(c, &p->d_Bext, bext_elems));
+  cudaMemsetAsync(p->d_Bext, 0, bext_elems * sizeof(float), c->stream);
+  TRYP(dev_alloc(c, &d_G, (size_t)nnb * per2 * cw));
+  cudaMemsetAsync(d_G, 0, (size_t)nnb * per2 * cw * sizeof(double), c->stream);
+  size_t smem = (size_t)n * npj * sizeof(double) * cw;
+  cudaError_t e;
+  if (c->cplx) {
+    e = cudaFuncSetAttribute(k_build_ext<double2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+      k_build_ext<double2><<<(unsigned)p->nchunks, 256, smem, c->stream>>>(
+          c->md, d_ec, p->d_ext_atom, c->d_atom_pair_start, c->d_pair_cell, (const double2*)c->d_Cd64, npj,
+          (const double2*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, NH, NT, p->d_Bext, (double2*)d_G);
+  } else {
+    e = cudaFuncSetAttribute(k_build_ext<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+      k_build_ext<double><<<(unsigned)p->nchunks, 256, smem, c->stream>>>(
+          c->md, d_ec, p->d_ext_atom, c->d_atom_pair_start, c->d_pair_cell, (const double*)c->d_Cd64, npj,
+          (const double*)c->d_H64, d_cps, d_cpi, c->d_pair_atom, p->d_nb_start, p->d_nb_atom, NH, NT, p->d_Bext, d_G);
   }
-  std::vector<double> G((size_t)nnb * npj * npj);
+  if (e == cudaSuccess) { c->launches++; e = cudaGetLastError(); }
+  std::vector<double> G((size_t)nnb * per2 * cw);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e == cudaSuccess) e = cudaMemcpy(G.data(), d_G, G.size() * sizeof(double), cudaMemcpyDeviceToHost);
   cleanup();
   if (e != cudaSuccess) { c->err = std::string("fused plan build: ") + cudaGetErrorString(e); return PAWFE_ECUDA; }
 #undef TRYP
-  // GD^{ab} = G^{ab} Delta^b_Sinv; cross-check the diagonal blocks against G^a of atoms_create
-  std::vector<float> GD((size_t)nnb * npj * npj);
-  const size_t per2 = (size_t)npj * npj;
+  // GD^{ab} = G^{ab} Delta^b_Sinv (complex arithmetic when cw = 2); cross-check the diagonal blocks against G^a of atoms_create
+  std::vector<float> GD((size_t)nnb * per2 * cw);
   for (int a = 0; a < natoms; ++a)
     for (int s = ns[a]; s < ns[a + 1]; ++s) {
       const int b = na[s];
-      const double* g = &G[(size_t)s * per2];
+      const double* g = &G[(size_t)s * per2 * cw];
       if (b == a) {
         double dmax = 0, gmax = 0;
-        for (size_t i = 0; i < per2; ++i) { dmax = std::max(dmax, std::fabs(g[i] - c->h_G[a * per2 + i])); gmax = std::max(gmax, std::fabs(g[i])); }
+        for (size_t i = 0; i < per2 * cw; ++i) { dmax = std::max(dmax, std::fabs(g[i] - c->h_G[a * per2 * cw + i])); gmax = std::max(gmax, std::fabs(g[i])); }
         if (dmax > 1e-9 * std::max(gmax, 1e-300)) { c->err = "fused plan: G^{aa} from the extension blocks disagrees with atoms_create"; return PAWFE_ECUDA; }
       }
-      const double* si = &c->h_dSinv[(size_t)b * per2];
+      const double* si = &c->h_dSinv[(size_t)b * per2 * cw];
       for (int i = 0; i < npj; ++i)
         for (int j = 0; j < npj; ++j) {
-          double t = 0;
-          for (int k = 0; k < npj; ++k) t += g[i * npj + k] * si[k * npj + j];
-          GD[(size_t)s * per2 + i * npj + j] = (float)t;
+          double tr = 0, ti = 0;
+          for (int k = 0; k < npj; ++k) {
+            const double gr = g[(i * npj + k) * cw], gi = cw == 2 ? g[(i * npj + k) * cw + 1] : 0.0;
+            const double sr = si[(k * npj + j) * cw], sim = cw == 2 ? si[(k * npj + j) * cw + 1] : 0.0;
+            tr += gr * sr - gi * sim; ti += gr * sim + gi * sr;
+          }
+          GD[((size_t)s * per2 + i * npj + j) * cw] = (float)tr;
+          if (cw == 2) GD[((size_t)s * per2 + i * npj + j) * cw + 1] = (float)ti;
         }
     }
   TRY(upload(c, &p->d_GD, GD));
@@ -507,7 +543,8 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   return PAWFE_OK;
 }
 
-pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int B) {
+pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int Bvec) {
+  const int B = Bvec * (c->cplx ? 2 : 1);   // real columns
   if (B <= p->Bcap) return PAWFE_OK;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64); cudaFree(p->d_Wcat_lo);
@@ -526,16 +563,40 @@ pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int B) {
 }
 
 // P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple)
+template <int NPJ>
+pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int Wr) {
+  const int n = c->n;
+  const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)NPJ * n * 2 + 3) / 4 * 16 + (size_t)NPJ * 128 * 4;
+  TRY(pawfe_ensure_smem(c, (const void*)k_projF<NPJ, true>, smem));
+  k_projF<NPJ, true><<<dim3((unsigned)c->npairs, ceil_div(Wr, 128)), 256, smem, c->stream>>>(
+      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw);
+  KERNEL_CHECK(c, "k_projF");
+  return PAWFE_OK;
+}
+
+// X: the block as floats (complex: interleaved), ldx in floats; B vectors.
 pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
   CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
+  if (c->cplx) {
+    switch (npj) {
+#define CASE_PC(N) case N: TRY(project_cplx<N>(c, p, X, ldx, 2 * B)); break;
+      CASE_PC(1) CASE_PC(2) CASE_PC(3) CASE_PC(4) CASE_PC(5) CASE_PC(6) CASE_PC(7) CASE_PC(8)
+      CASE_PC(9) CASE_PC(10) CASE_PC(11) CASE_PC(12) CASE_PC(13) CASE_PC(14) CASE_PC(15) CASE_PC(16)
+#undef CASE_PC
+    }
+    k_couple<float2><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
+        npj, mode, (const float2*)p->d_P1, p->ldw / 2, B, (const float2*)c->d_dSinv32, (const float2*)c->d_D32, p->d_nb_start,
+        p->d_nb_atom, (const float2*)p->d_GD, (float2*)p->d_Wcat, p->ldw / 2);
+    KERNEL_CHECK(c, "k_couple");
+    return PAWFE_OK;
+  }
   size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4;
   dim3 grid((unsigned)c->npairs, ceil_div(B, 128));
 #define LAUNCH_PROJ2(NPJ)                                                                                            \
   do {                                                                                                               \
-    static size_t smem_attr = 0;                                                                                     \
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj2<NPJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; } \
+    TRY(pawfe_ensure_smem(c, (const void*)k_proj2<NPJ>, smem)); \
     k_proj2<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw); \
   } while (0)
   switch (npj) {
@@ -548,7 +609,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   }
 #undef LAUNCH_PROJ2
   KERNEL_CHECK(c, "k_proj2");
-  k_couple<<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
+  k_couple<float><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
       npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
       p->d_GD, p->d_Wcat, p->ldw);
   KERNEL_CHECK(c, "k_couple");
@@ -564,8 +625,7 @@ pawfe_status setup_nonlocal64_t(pawfe_ctx* c, FusedPlan* p, const float* X, long
   dim3 grid((unsigned)c->npairs, ceil_div(B, 64));
   {
     const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8 + (size_t)NPJ * 64 * 8;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_proj64<NPJ, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    TRY(pawfe_ensure_smem(c, (const void*)k_proj64<NPJ, float>, smem));
     k_proj64<NPJ, float><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const double*)c->d_Cd64, X, ldx, B, p->d_P64, p->ldw);
     KERNEL_CHECK(c, "k_proj64");
   }
@@ -574,8 +634,7 @@ pawfe_status setup_nonlocal64_t(pawfe_ctx* c, FusedPlan* p, const float* X, long
   KERNEL_CHECK(c, "k_couple64");
   {
     const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatter64<NPJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    TRY(pawfe_ensure_smem(c, (const void*)k_scatter64<NPJ>, smem));
     k_scatter64<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const double*)c->d_Cd64, p->d_W64, p->ldw, B, Y, ldy);
     KERNEL_CHECK(c, "k_scatter64");
   }
@@ -605,7 +664,7 @@ void fused_invalidate(pawfe_ctx* c) {
 }
 
 bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
-  return (prec == PAWFE_TF32 || prec == PAWFE_FP32) && !c->cplx && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
+  return (prec == PAWFE_TF32 || (prec == PAWFE_FP32 && !c->cplx)) && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
 }
 
 // run `body` on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream
@@ -677,41 +736,66 @@ pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long l
     TRY(dev_alloc(c, &p->d_xlo, (size_t)c->M * ldx));
     p->xlo_elems = (size_t)c->M * ldx;
   }
+  const int Wr = B * (c->cplx ? 2 : 1);   // X, Y as float blocks: ldx, ldy in floats, Wr real columns
   TRY(project_and_couple(c, p, X, ldx, B, 2));
-  if (ldy == B) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * B * sizeof(float), c->stream));
-  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)B * sizeof(float), c->M, c->stream));
-  return cell_pass(c, p, prec, X, ldx, Y, ldy, B, 1.0f, 0, p->d_xlo);
+  if (ldy == Wr) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * Wr * sizeof(float), c->stream));
+  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)Wr * sizeof(float), c->M, c->stream));
+  return cell_pass(c, p, prec, X, ldx, Y, ldy, Wr, 1.0f, 0, p->d_xlo);
 }
 
-pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds, const double* as, const double* acs,
-                               const double* zzs, double z_over_e, float* X, long ld, int B, void* workspace) {
+// recovery's low-rank part for complex contexts:  X -= M_D^-1 C W  (W = rows [0, npj) of Wcat)
+template <int NPJ>
+static pawfe_status scatter_cplx(pawfe_ctx* c, FusedPlan* p, float* X, long ldx, int Wr) {
+  const int n = c->n;
+  const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)NPJ * n * 2 + 3) / 4 * 16;
+  TRY(pawfe_ensure_smem(c, (const void*)k_scatterF<NPJ, true>, smem));
+  k_scatterF<NPJ, true><<<dim3((unsigned)c->npairs, ceil_div(Wr, 128)), 256, smem, c->stream>>>(
+      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, p->d_Wcat, p->ldw, 32, Wr, 1, -1.0f, X, ldx);
+  KERNEL_CHECK(c, "k_scatterF");
+  return PAWFE_OK;
+}
+
+// X: the block in the context's FP32 storage scalar (float, or float2 interleaved), ld and B in those scalars.  Inside, every
+// array is a real block of Wr = B * cw columns (cw = 2 for complex contexts) with leading dimension ldw = roundup4(Wr).
+pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds, const double* as, const double* acs,
+                          const double* zzs, double z_over_e, void* Xv, long ld, int B, void* workspace) {
   TRY(fused_prepare(c, B));
   FusedPlan* p = (FusedPlan*)c->fused;
+  const int cw = c->cplx ? 2 : 1;
+  const int Wr = B * cw;
+  float* X = (float*)Xv;
+  const long ldx = ld * cw;
   // workspace arrays use this block's own padded leading dimension; P1 / Wcat use the plan's (widest block seen)
-  const long ldw = roundup4(B);
+  const long ldw = roundup4(Wr);
   const size_t blk_s = ((size_t)c->M * ldw * 4 + 255) / 256 * 256, blk_d = ((size_t)c->M * ldw * 8 + 255) / 256 * 256;
   char* ws = (char*)workspace;
   double* Yt = (double*)ws;
   float* RX = (float*)(ws + blk_d);
   float* RY = (float*)(ws + blk_d + blk_s);
   float* XLO = (float*)(ws + blk_d + 2 * blk_s);   // FP32 mode only (pawfe_filter_workspace adds the block)
-  // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda, fused (setup_fp64.cuh): S X is never stored ----
-  CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
-  FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
-  TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
-  {
-    StreamSwap sw(c, p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
-    const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_mass_sf<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
-    k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
-        c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
-    KERNEL_CHECK(c, "k_mass_sf");
-    if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
+  // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda; S X is never stored ----
+  if (c->cplx) {
+    // complex: the generic FP64 applies (DMMA cell product, mass sweeps, Ritz values folded into the coupling)
+    TRY((pawfe_apply_HS<float2, double2, double2>(c, 0, false, (const float2*)X, ld, (double2*)Yt, ldw / 2, B)));
+    TRY((pawfe_sub_SX_lambda<float2, double2>(c, (const float2*)X, ld, (double2*)Yt, ldw / 2, B, ds, ds + (size_t)(m + 1) * B)));
+  } else {
+    // real: fused (setup_fp64.cuh)
+    CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
+    FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
+    TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
+    {
+      StreamSwap sw(c, p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
+      const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
+      TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float>, smem));
+      k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
+          c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
+      KERNEL_CHECK(c, "k_mass_sf");
+      if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
+    }
+    JOIN_AUX(c, p);
   }
-  JOIN_AUX(c, p);
   const int gs = 8 * c->sm_count;
-  k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, Yt, z_over_e, RX, RY);
+  k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
   const long nquads = c->M * (ldw / 4);
@@ -719,20 +803,26 @@ pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const doubl
     FORK_AUX(c, p);
     { StreamSwap sw(c, p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
     k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
-                                         ds + (size_t)(th - 1) * B, B, (float)acs[th], (float)zzs[th]);
+                                         ds + (size_t)(th - 1) * B, Wr, cw, (float)acs[th], (float)zzs[th]);
     KERNEL_CHECK(c, "k_prepass");
     JOIN_AUX(c, p);
-    TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, B, (float)as[th], 1, XLO));
+    TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, XLO));
     std::swap(RX, RY);
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----
   TRY(project_and_couple(c, p, RY, ldw, B, 1));
-  k_recover2<<<gs, 256, 0, c->stream>>>(c->md, ldw, B, RY, X, ld, ds + (size_t)m * B);
+  k_recover2<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
   KERNEL_CHECK(c, "k_recover2");
-  if (c->npairs > 0) {
+  if (c->npairs > 0 && c->cplx) {
+    switch (c->npj) {
+#define CASE_SC(N) case N: TRY(scatter_cplx<N>(c, p, X, ldx, Wr)); break;
+      CASE_SC(1) CASE_SC(2) CASE_SC(3) CASE_SC(4) CASE_SC(5) CASE_SC(6) CASE_SC(7) CASE_SC(8)
+      CASE_SC(9) CASE_SC(10) CASE_SC(11) CASE_SC(12) CASE_SC(13) CASE_SC(14) CASE_SC(15) CASE_SC(16)
+#undef CASE_SC
+    }
+  } else if (c->npairs > 0) {
     size_t smem = (size_t)c->n * 12 + (size_t)c->npj * c->n * 4;
-    static size_t smem_attr = 0;
-    if (smem > smem_attr) { CUDA_TRY(c, cudaFuncSetAttribute(k_scatter2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_attr = smem; }
+    TRY(pawfe_ensure_smem(c, (const void*)k_scatter2, smem));
     k_scatter2<<<dim3((unsigned)c->npairs, ceil_div(B, 128)), 256, smem, c->stream>>>(
         c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, c->npj, p->d_Wcat, p->ldw, B, -1.0f, X, ld);
     KERNEL_CHECK(c, "k_scatter2");

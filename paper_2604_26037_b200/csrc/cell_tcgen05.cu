@@ -287,7 +287,7 @@ k_cell_tcgen05(const TcArgs a) {
             // both operand streams are stored pre-swizzled and block-contiguous: one linear bulk copy per chunk
             const float* src = (c < a.kchunks)
                 ? a.H32t + ((long)((cell * a.NH + half) * a.kchunks + c) * a.NT) * 32 * a.ncomp
-                : a.Bext + ((long)(ext0 + c - a.kchunks) * a.NH + half) * a.NT * 32;
+                : a.Bext + ((long)(ext0 + c - a.kchunks) * a.NH + half) * a.NT * 32 * a.ncomp;
             if (a.dbg & 64) { ptx::bulk_load(dst, src, (uint32_t)bbytes / 2, &full[s]); ptx::bulk_load(dst + bbytes / 2, src, (uint32_t)bbytes / 2, &full[s]); }
             else ptx::bulk_load(dst, src, (uint32_t)bbytes, &full[s]);
           }

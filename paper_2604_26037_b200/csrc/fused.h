@@ -1,4 +1,4 @@
-// fused.h -- the fused Chebyshev step of Algorithm 2 for real FP32-storage blocks.
+// fused.h -- the fused Chebyshev step of Algorithm 2 for FP32-storage blocks (real or complex).
 //
 // One step  R_X <- a H S^-1approx R_Y - a c R_Y - zeta zeta1 R_X + a Y Lambda_Y  is computed without ever
 // writing T = S^-1approx R_Y or H T to memory:
@@ -23,12 +23,14 @@ void fused_invalidate(pawfe_ctx* c);
 // The couplings D changed: nothing to rebuild (D is read at run time), kept for symmetry.
 bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B);
 
-// Algorithm 2 for a real context in FP32 storage with the tcgen05 contraction: PAWFE_TF32 (one TF32 pass) or PAWFE_FP32
-// (three passes on hi/lo operand splits, FP32-accurate).  Coefficients come from
-// pawfe_filter_scalars (api_filter.cu).  X: [dof][vec] float, ld >= B.  workspace as pawfe_filter_workspace.
-pawfe_status fused_filter_real(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds /*device scalars*/, const double* as,
-                               const double* acs, const double* zzs, double z_over_e, float* X, long ld, int B,
-                               void* workspace);
+// Algorithm 2 in FP32 storage with the tcgen05 contraction: PAWFE_TF32 (one TF32 pass; real and complex contexts) or
+// PAWFE_FP32 (real contexts: three passes on hi/lo operand splits, FP32-accurate).  Coefficients come from
+// filter_scalars (api_filter.cu).  X: [dof][vec] float (real) or float2 (complex), ld >= B in those scalars; complex
+// blocks need B and ld even and a 16-byte aligned X.  workspace as pawfe_filter_workspace.
+pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds /*device scalars*/, const double* as,
+                          const double* acs, const double* zzs, double z_over_e, void* X, long ld, int B,
+                          void* workspace);
 
-// Y = H X (TF32 contraction, non-local term through the K-extension).  X, Y float, 16-byte aligned, ld % 4 == 0.
+// Y = H X (tcgen05 contraction, non-local term through the K-extension).  X, Y as float blocks (complex: interleaved,
+// ldx / ldy in floats), 16-byte aligned, ldx % 4 == ldy % 4 == 0; B vectors.
 pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B);

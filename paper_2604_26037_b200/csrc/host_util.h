@@ -25,6 +25,11 @@ static inline pawfe_status upload(pawfe_ctx* ctx, T** d, const std::vector<T>& h
   return PAWFE_OK;
 }
 
+// Raise (never lower) a kernel's dynamic shared-memory limit to `bytes`.  One table for the whole library: a template
+// kernel instantiated in several translation units is ONE function to the runtime, so per-unit bookkeeping would let
+// one unit lower what another has raised.  func: the kernel's host address.
+pawfe_status pawfe_ensure_smem(pawfe_ctx* c, const void* func, size_t bytes);
+
 void pawfe_free_mesh(pawfe_ctx* c);
 void pawfe_free_pot(pawfe_ctx* c);
 void pawfe_free_atoms(pawfe_ctx* c);

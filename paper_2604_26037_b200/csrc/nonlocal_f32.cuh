@@ -1,7 +1,7 @@
 // nonlocal_f32.cuh -- pair-parallel kernels of the non-local PAW terms (Fig. 2 steps ii-iii; Eq. 16,
 // Eq. 28) for FP32 storage, real or complex (interleaved) blocks seen as Wr = B * cw real columns:
 //   k_projF   :  P[a][al][.] += sum_I Cd[pair][al][I] * (s_I X[J(e,I)][.])        Cd = rows of C^{e,a dagger} (Eq. 34)
-//   k_scatterF:  Y[J(e,I)][.] += s_I * sum_al conj(Cd[pair][al][I]) * W[a][al][.]
+//   k_scatterF:  Y[J(e,I)][.] += scale * s_I * sum_al conj(Cd[pair][al][I]) * W[a][al][.]     (W rows: [a][wrows][ldp])
 // with s_I = M_D^-1 at the node when the scale flag is set (S^-1approx, Eq. 28), else 1.  One CTA per (cell, atom)
 // pair and 128 real columns; 8 warps over the cell's rows, one 16-byte piece per lane; four loads in flight per thread.
 #pragma once
@@ -87,7 +87,8 @@ k_projF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
 template <int NPJ, bool CPLX>
 __global__ void __launch_bounds__(256, (NPJ <= 9 ? 3 : 2))
 k_scatterF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom, const float* __restrict__ Cd,
-           const float* __restrict__ W, long ldp /*floats*/, int Wr, int out_scale, float* __restrict__ Y, long ldy /*floats*/) {
+           const float* __restrict__ W, long ldp /*floats*/, int wrows /*rows of W per atom*/, int Wr, int out_scale, float scale,
+           float* __restrict__ Y, long ldy /*floats*/) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int cw = CPLX ? 2 : 1;
   const int n = md.n, n1 = md.n1;
@@ -102,7 +103,7 @@ k_scatterF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict_
     long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
     const double mi = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
     nodeO[I] = (mi == 0.0) ? -1 : J * ldy * 4;
-    nodeS[I] = out_scale ? (float)mi : 1.f;
+    nodeS[I] = scale * (out_scale ? (float)mi : 1.f);
   }
   for (int i = threadIdx.x; i < NPJ * n * cw; i += blockDim.x) Cs[i] = Cd[(long)pr * NPJ * n * cw + i];
   __syncthreads();
@@ -111,7 +112,7 @@ k_scatterF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict_
   if (v >= Wr) return;
   float4 wv[NPJ];
 #pragma unroll
-  for (int al = 0; al < NPJ; ++al) wv[al] = *reinterpret_cast<const float4*>(W + ((long)a * NPJ + al) * ldp + v);
+  for (int al = 0; al < NPJ; ++al) wv[al] = *reinterpret_cast<const float4*>(W + ((long)a * wrows + al) * ldp + v);
   char* yv = reinterpret_cast<char*>(Y + v);
   for (int I = w; I < n; I += 8) {
     const long off = nodeO[I];

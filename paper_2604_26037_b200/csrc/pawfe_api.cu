@@ -9,8 +9,21 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
+#include <mutex>
 
 using namespace pawfe;
+
+pawfe_status pawfe_ensure_smem(pawfe_ctx* c, const void* func, size_t bytes) {
+  static std::mutex mu;
+  static std::map<const void*, size_t> limit;   // per kernel: the limit set so far (default 48 KB needs no call)
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& cur = limit[func];
+  if (bytes <= cur || bytes <= 48 * 1024) return PAWFE_OK;
+  CUDA_TRY(c, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  cur = bytes;
+  return PAWFE_OK;
+}
 
 void pawfe_free_mesh(pawfe_ctx* c) {
   cudaFree(c->d_md1); c->d_md1 = nullptr;

@@ -251,3 +251,59 @@ def test_filter_ragged_block_width(B):
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
     assert _relerr(_to_host(Xd, False), want) < 5e-2
+
+
+@pytest.mark.parametrize("name,B", [("cfg2_twin", 136), ("cfg3_twin", 80), ("cfg4_twin", 256)])
+@pytest.mark.parametrize("prec", ["tf32", "fp32"])
+def test_apply_H_wide_blocks(name, B, prec):
+    """Block widths that need two or more 128-column tiles on the twins: p = 7 (two node halves of 256 columns, both
+    TMEM buffers full), complex (P / Q accumulators, 160 real columns), Dirichlet with the full config-4 width."""
+    from paper_2604_26037_b200 import PREC
+    cfg, sysd, ops, ctx = _setup(name)
+    X = random_block(cfg, B, stream=31) * ops.mask[:, None]
+    Xd = _to_dev(X, prec, cfg.complex)
+    Yd = torch.full_like(Xd, float("nan"))
+    ctx.apply_H(PREC[prec], Xd, Yd, B, B)
+    torch.cuda.synchronize()
+    want = ops.apply_H(X) * ops.mask[:, None]
+    assert _relerr(_to_host(Yd, cfg.complex), want) < TOL[prec], (name, prec)
+
+
+@pytest.mark.parametrize("name,B", [("cfg2_twin", 136), ("cfg3_twin", 80)])
+def test_filter_wide_blocks(name, B):
+    from oracle import chfsi
+    from paper_2604_26037_b200 import TF32
+    cfg, sysd, ops, ctx = _setup(name)
+    m = 4
+    X0 = random_block(cfg, B, stream=33) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+    Xd = _to_dev(X, "tf32", cfg.complex)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, cfg.complex), want) < 5e-2
+
+
+def test_filter_complex_odd_width_generic_sequence():
+    """A complex block of odd width cannot be cut into 16-byte pieces of interleaved columns: the library runs the
+    unfused sequence (and asks for its larger workspace); the result is the same filter."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import TF32
+    cfg, sysd, ops, ctx = _setup("cfg3_twin")
+    B, m = 7, 4
+    X0 = random_block(cfg, B, stream=35) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+    Xd = _to_dev(X, "tf32", True)
+    nbytes = ctx.filter_workspace(TF32, B)
+    assert nbytes > ctx.filter_workspace(TF32, B + 1)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, True), want) < 5e-2
