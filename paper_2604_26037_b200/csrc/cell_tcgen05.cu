@@ -18,6 +18,7 @@
 // TMEM owner.  Pipelines: full[s] / empty[s] per shared-memory stage, accum_full[b] / accum_empty[b] per
 // accumulator buffer (two buffers: the epilogue of one vector tile runs under the MMAs of the next).
 #include "cell_tcgen05.h"
+#include "host_util.h"
 #include "ptx_sm100.cuh"
 #include <cstdio>
 #include <cstdlib>
@@ -28,8 +29,14 @@ namespace {
 constexpr int kChunkK = 32;             // K rows per pipeline stage (= 128 bytes of a K-major tf32 row)
 constexpr int kTileV = 128;             // vectors per MMA (M)
 constexpr int kABytes = kChunkK * kTileV * 4;  // 16 KB per vector tile and stage
-constexpr int kThreads = 320;           // warps 0-3 epilogue, 4-7 gather, 8 TMA, 9 MMA / TMEM owner
-constexpr int kMaxStages = 6;
+constexpr int kEpiWarps = 8;            // two per TMEM lane quadrant (warp % 4), alternating column groups: the assembly is a
+                                        // chain of dependent TMEM / shared / global operations, two warps per scheduler overlap it
+constexpr int kEpiThreads = 32 * kEpiWarps;
+constexpr int kGatherWarps = 4;
+constexpr int kGatherThreads = 32 * kGatherWarps;
+constexpr int kWarpTma = kEpiWarps + kGatherWarps, kWarpMma = kWarpTma + 1;
+constexpr int kThreads = 32 * (kWarpMma + 1);   // warps 0-7 epilogue, 8-11 gather, 12 TMA, 13 MMA / TMEM owner
+constexpr int kMaxStages = 8;
 
 struct TcArgs {
   MeshDev md;
@@ -78,55 +85,85 @@ __global__ void k_retile_h32(const float* __restrict__ H, int n, int ldk, int NH
   }
 }
 
-__device__ __forceinline__ void bar_sync_128(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void bar_sync_epi(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(kEpiThreads) : "memory"); }
+__device__ __forceinline__ void bar_sync_gather(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(kGatherThreads) : "memory"); }
 
 // Persistent CTAs (one per SM) loop over tiles (cell, node half); inside a tile over the vector tiles of 128
-// ("subtiles").  The first vector tile of a tile streams its H^e half from HBM, the following ones re-read it
-// from L2.  Accumulators are double-buffered in tensor memory (subtile parity), so the assembly epilogue of one
+// ("subtiles").  Accumulators are double-buffered in tensor memory (subtile parity), so the assembly epilogue of one
 // subtile runs under the loads and MMAs of the next.  Roles are decoupled through mbarriers only.
+//   PAIR = false: one CTA per tile; the first vector tile streams its H^e half from HBM, the following ones re-read it
+//     from L2.
+//   PAIR = true (blocks wider than 128 columns): the two CTAs of a cluster (one TPC) work on the same tile with
+//     tcgen05.mma.cta_group::2, M = 256: CTA r gathers and assembles vector tile 2j + r and loads only rows
+//     [r NT/2, (r+1) NT/2) of every matrix block, so each H^e block crosses L2 -> SM once per pair instead of once per
+//     vector tile.  The leader (rank 0) issues the MMAs for both; rank 1's owner warp forwards "stage full" to it.
+template <bool PAIR, bool CPLX>
 __global__ void __launch_bounds__(kThreads, 1)
 k_cell_tcgen05(const TcArgs a) {
+  constexpr int ncomp = CPLX ? 2 : 1;   // complex: two matrix blocks (Re, Im) per stage and two accumulators per buffer
   extern __shared__ __align__(1024) uint8_t smem[];
-  const int bbytes1 = a.NT * 128;                       // one matrix block (Re or Im)
-  const int bbytes = a.ncomp * bbytes1;
+  const int bbytes1 = (PAIR ? a.NT / 2 : a.NT) * 128;   // this CTA's rows of one matrix block (Re or Im)
+  const int bbytes = ncomp * bbytes1;
   const int sbytes = kABytes + bbytes;                  // one stage: [A][B (Re)][B (Im)]
-  long* gJ = reinterpret_cast<long*>(smem + a.stages * sbytes);           // [NH * NT] gather rows: byte offset or -1
-  long* eJ = gJ + a.NH * a.NT;                                            // [NT] output rows of this half
+  int* gR = reinterpret_cast<int*>(smem + a.stages * sbytes);             // [kchunks * 32] gather rows: node index or -1
+  long* eJ = reinterpret_cast<long*>(gR) + a.NH * a.NT;                   // [NT] output rows of this half
   float* eS = reinterpret_cast<float*>(eJ + a.NT);                        // [NT] output scale
-  float* stage_epi = eS + a.NT;                                           // [4 warps][32 nodes][32 vectors]
-  uint64_t* full = reinterpret_cast<uint64_t*>(stage_epi + 4 * 32 * 32);  // [stages]
+  float* stage_epi = eS + a.NT;                                           // [epilogue warps][32 nodes][32 vectors]
+  uint64_t* full = reinterpret_cast<uint64_t*>(stage_epi + kEpiWarps * 32 * 32);  // [stages]
   uint64_t* empty = full + kMaxStages;                                    // [stages]
-  uint64_t* accum_full = empty + kMaxStages;                              // [2]
+  uint64_t* full_peer = empty + kMaxStages;                               // [stages] leader: rank 1's stage is full
+  uint64_t* accum_full = full_peer + kMaxStages;                          // [2]
   uint64_t* accum_empty = accum_full + 2;                                 // [2]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_empty + 2);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // the shuffle tells the compiler that the warp index is warp-uniform: role branches become uniform branches and the
+  // operands computed inside them can live in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+  const uint32_t rank = PAIR ? ptx::cluster_ctarank() : 0u;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < a.stages; ++s) { ptx::mbar_init(&full[s], 128 + 1); ptx::mbar_init(&empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { ptx::mbar_init(&accum_full[b], 1); ptx::mbar_init(&accum_empty[b], 128); }
+    for (int s = 0; s < a.stages; ++s) { ptx::mbar_init(&full[s], kGatherThreads + 1); ptx::mbar_init(&empty[s], 1); ptx::mbar_init(&full_peer[s], 1); }
+    // accum_empty: PAIR: one arrival per epilogue warp of both CTAs, on the leader's barrier
+    for (int b = 0; b < 2; ++b) { ptx::mbar_init(&accum_full[b], 1); ptx::mbar_init(&accum_empty[b], PAIR ? 2 * kEpiWarps : kEpiThreads); }
     ptx::fence_barrier_init();
   }
-  if (warp == 9) ptx::tmem_alloc(tmem_slot, a.tmem_cols);
+  if (PAIR) ptx::cluster_sync();   // both CTAs' barriers exist before any remote arrival or multicast commit
+  if (warp == kWarpMma) { if (PAIR) ptx::tmem_alloc_pair(tmem_slot, a.tmem_cols); else ptx::tmem_alloc(tmem_slot, a.tmem_cols); }
   ptx::tc_fence_before_sync();
   __syncthreads();
   ptx::tc_fence_after_sync();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);
   const int n1 = a.md.n1;
+  const int nsub = PAIR ? (a.nvt + 1) / 2 : a.nvt;   // subtiles per tile; subtile j of CTA r is vector tile 2j + r (PAIR) or j
+  // 32-bit shared-memory addresses of the stage ring and the barriers (8 bytes per barrier)
+  const uint32_t sm0 = ptx::smem_u32(smem);
+  const uint32_t full_a = ptx::smem_u32(full), empty_a = ptx::smem_u32(empty), fpeer_a = ptx::smem_u32(full_peer);
+  const uint32_t accf_a = ptx::smem_u32(accum_full), acce_a = ptx::smem_u32(accum_empty);
+  // gather threads: local (a, b, c) of the up to four cell nodes whose row index this thread computes per tile
+  constexpr int kDec = 512 / kGatherThreads;   // n <= 512
+  int gdec[kDec];
+  for (int k = 0; k < kDec; ++k) gdec[k] = -1;
+  if (warp >= kEpiWarps && warp < kWarpTma) {
+    for (int k = 0; k < kDec; ++k) {
+      const int I = (int)threadIdx.x - kEpiThreads + kGatherThreads * k;
+      if (I < a.n) gdec[k] = (I / (n1 * n1)) | (((I / n1) % n1) << 8) | ((I % n1) << 16);
+    }
+  }
 
-  uint32_t it = 0;        // running chunk counter (same sequence in every role)
-  uint32_t sub_iter = 0;  // running subtile counter: accumulator buffer = sub_iter & 1
-  for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+  uint32_t st_s = 0, st_ph = 0;   // running stage index and phase of this role's walk over the ring (same sequence in every role)
+  uint32_t sub_iter = 0;          // running subtile counter: accumulator buffer = sub_iter & 1
+  for (int tile = PAIR ? blockIdx.x >> 1 : blockIdx.x; tile < a.ntiles; tile += PAIR ? gridDim.x >> 1 : gridDim.x) {
     const int cell = tile / a.NH;
     const int half = tile - cell * a.NH;
-    const int ext0 = a.ext_start ? a.ext_start[cell] : 0;
-    const int nchunks = a.kchunks + (a.ext_start ? a.ext_start[cell + 1] - ext0 : 0);
+    // (values read from memory are made warp-uniform explicitly, see the note on `warp`)
+    const int ext0 = __shfl_sync(0xffffffffu, a.ext_start ? a.ext_start[cell] : 0, 0);
+    const int nchunks = a.kchunks + __shfl_sync(0xffffffffu, a.ext_start ? a.ext_start[cell + 1] - ext0 : 0, 0);
     int cx, cy, cz;
     mesh_cell_coords(a.md, cell, &cx, &cy, &cz);
 
-    if (warp < 4) {
+    if (warp < kEpiWarps) {
       // ================= epilogue: TMEM -> scaled vector reductions into Y (assembly, Fig. 2 step iv) =================
-      bar_sync_128(2);   // previous tile's readers of eJ / eS are done
-      for (int I = threadIdx.x; I < a.NT; I += 128) {
+      bar_sync_epi(2);   // previous tile's readers of eJ / eS are done
+      for (int I = threadIdx.x; I < a.NT; I += kEpiThreads) {
         const int Ig = half * a.NT + I;
         long J = -1;
         float sc = 0.f;
@@ -139,27 +176,29 @@ k_cell_tcgen05(const TcArgs a) {
         }
         eJ[I] = J; eS[I] = sc;
       }
-      bar_sync_128(2);
+      bar_sync_epi(2);
       const int ncols = min(a.NT, a.n - half * a.NT);
       // Each warp owns 32 vectors (TMEM lanes).  32 output nodes at a time: TMEM -> registers (lane = vector) ->
       // scaled -> staging tile [node][vector] in shared memory -> each thread takes 4 consecutive vectors of one
       // node and issues ONE 16-byte vector reduction (REDG.128): 4x fewer atomic lane-operations than scalar adds.
       float* stg = stage_epi + warp * (32 * 32);
+      const int quad = warp & 3, grp = warp >> 2;   // TMEM lanes [32 quad, 32 quad + 32); column groups grp, grp + 2, ...
       const int sub = lane >> 3, v4 = (lane & 7) * 4;
-      for (int vt = 0; vt < a.nvt; ++vt) {
-        const uint32_t buf = (sub_iter + vt) & 1, use = (sub_iter + vt) >> 1;
+      for (int j = 0; j < nsub; ++j) {
+        const uint32_t buf = (sub_iter + j) & 1, use = (sub_iter + j) >> 1;
         ptx::mbar_wait(&accum_full[buf], use & 1);
         ptx::tc_fence_after_sync();
-        const int vb = vt * kTileV + warp * 32;
+        const int vt = PAIR ? 2 * j + (int)rank : j;
+        const int vb = vt * kTileV + quad * 32;
         const bool vok = vb + v4 < a.B;             // B % 4 == 0: a float4 is all in or all out
         char* yv = reinterpret_cast<char*>(a.Y + vb + v4);
-        if (vb < a.B && !(a.dbg & 16) && a.ncomp == 2) {
+        if (vb < a.B && !(a.dbg & 16) && CPLX) {
           // complex: columns are interleaved (re, im); with P = X^T Hr^T and Q = X^T Hi^T,
           //   Y_re = P_re - Q_im,  Y_im = P_im + Q_re  ->  y = P + (lane odd ? +1 : -1) * Q of the partner lane
           const float sg = (lane & 1) ? 1.f : -1.f;
-          for (int col0 = 0; col0 < ncols; col0 += 16) {
+          for (int col0 = 16 * grp; col0 < ncols; col0 += 16 * (kEpiWarps / 4)) {
             uint32_t r[16], q[16];
-            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
+            const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
             ptx::tmem_ld16(taddr, r);
             ptx::tmem_ld16(taddr + a.NT, q);
             ptx::tmem_ld_wait();
@@ -188,9 +227,9 @@ k_cell_tcgen05(const TcArgs a) {
             __syncwarp();
           }
         } else if (vb < a.B && !(a.dbg & 16)) {
-          for (int col0 = 0; col0 < ncols; col0 += 32) {
+          for (int col0 = 32 * grp; col0 < ncols; col0 += 32 * (kEpiWarps / 4)) {
             uint32_t r[32];
-            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
+            const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * a.acc_stride + (uint32_t)col0;
             ptx::tmem_ld16(taddr, *reinterpret_cast<uint32_t(*)[16]>(&r[0]));
             if (col0 + 16 < ncols) ptx::tmem_ld16(taddr + 16, *reinterpret_cast<uint32_t(*)[16]>(&r[16]));
             ptx::tmem_ld_wait();
@@ -224,115 +263,186 @@ k_cell_tcgen05(const TcArgs a) {
           }
         }
         ptx::tc_fence_before_sync();
-        ptx::mbar_arrive(&accum_empty[buf]);
-      }
-    } else if (warp < 8) {
-      // ================= gather producers: X rows -> swizzled MN-major A tiles (Fig. 2 step i) =================
-      const int t = threadIdx.x - 128;  // 0..127
-      bar_sync_128(1);   // previous tile's readers of gJ are done
-      for (int I = t; I < a.NH * a.NT; I += 128) {
-        long J = -1;
-        if (I < a.n) {
-          int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
-          J = mesh_node(a.md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-          J = (a.md.mdinv1[0][ix] * a.md.mdinv1[1][iy] * a.md.mdinv1[2][iz] == 0.0) ? -1 : J * a.ldx * 4;  // byte offset
+        if (PAIR) {
+          __syncwarp();
+          if (lane == 0) { if (rank == 0) ptx::mbar_arrive(&accum_empty[buf]); else ptx::mbar_arrive_remote(&accum_empty[buf], 0); }
+        } else {
+          ptx::mbar_arrive(&accum_empty[buf]);
         }
-        gJ[I] = J;
       }
-      bar_sync_128(1);
-      // per-thread constants: this thread always copies 16-byte column `lane` of rows wg, wg + 4, ... of a chunk
-      const int wg = t >> 5;                               // row within each group of 4
+    } else if (warp < kWarpTma) {
+      // ================= gather producers: X rows -> swizzled MN-major A tiles (Fig. 2 step i) =================
+      // (the loops of the three producer / issuer roles are kept lean: one warp per scheduler runs them, so every
+      //  dependent instruction costs its full latency; stage index and phase are running counters, shared-memory
+      //  addresses are 32-bit values computed once, and the row indices of a chunk are read before the wait)
+      const int t = threadIdx.x - kEpiThreads;  // 0 .. kGatherThreads - 1
+      bar_sync_gather(1);   // previous tile's readers of gR are done
+      for (int k = 0; k < kDec; ++k) {
+        const int I = t + kGatherThreads * k;
+        if (I >= a.kchunks * kChunkK) break;
+        int J = -1;
+        if (gdec[k] >= 0) {
+          int ix = cx * a.md.p + (gdec[k] & 0xff), iy = cy * a.md.p + ((gdec[k] >> 8) & 0xff), iz = cz * a.md.p + (gdec[k] >> 16);
+          bool masked = false;
+          if (a.md.periodic) {
+            if (ix >= a.md.N[0]) ix -= a.md.N[0];
+            if (iy >= a.md.N[1]) iy -= a.md.N[1];
+            if (iz >= a.md.N[2]) iz -= a.md.N[2];
+          } else {   // Dirichlet walls: the rows where M_D^-1 is stored as 0
+            masked = ix == 0 || iy == 0 || iz == 0 || ix == a.md.N[0] - 1 || iy == a.md.N[1] - 1 || iz == a.md.N[2] - 1;
+          }
+          if (!masked) J = (ix * a.md.N[1] + iy) * a.md.N[2] + iz;
+        }
+        gR[I] = J;
+      }
+      bar_sync_gather(1);
+      // per-thread constants: this thread always copies 16-byte column `lane` of rows wg, wg + 8, ... of a chunk
+      constexpr int kRows = kChunkK / kGatherWarps;        // rows of a chunk per thread
+      const int wg = t >> 5;                               // first row; wg % 4 is the row's place in its group of 4
       const int vl = lane * 4;                             // first vector of the 16-byte piece inside the tile
       // MN-major tf32 layout (128-byte swizzle, 32-byte atoms): 32-vector column block cb at cb * 4096; row r at
       // r * 128; its four 32-byte chunks q stored at q ^ (r % 4); r % 4 == wg for every row this thread copies
-      const uint32_t dst_thread = (lane >> 3) * 4096 + wg * 128 + (((((lane & 7) >> 1) ^ wg) << 5) | ((lane & 1) << 4));
-      uint32_t itc = it;
-      for (int vt = 0; vt < a.nvt; ++vt) {
+      const uint32_t dst_thread = sm0 + (lane >> 3) * 4096 + wg * 128 + (((((lane & 7) >> 1) ^ (wg & 3)) << 5) | ((lane & 1) << 4));
+      const long ldx4 = a.ldx * 4;
+      for (int j = 0; j < nsub; ++j) {
+        const int vt = PAIR ? 2 * j + (int)rank : j;
         const int v = vt * kTileV + vl;
         const bool vok = v < a.B;
         const char* xv = reinterpret_cast<const char*>(a.X + v);
-        for (int c = 0; c < nchunks; ++c, ++itc) {
-          const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
-          ptx::mbar_wait(&empty[s], ph ^ 1);
-          const uint32_t abase = ptx::smem_u32(smem + s * sbytes) + dst_thread;
-          if (c < a.kchunks) {
-            const long* offs = gJ + c * kChunkK + wg;
+        const int* rows_t = gR + wg;
+        for (int c = 0; c < a.kchunks; ++c, rows_t += kChunkK) {
+          int rows[kRows];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const long off = (c * kChunkK + wg + 4 * i < a.NH * a.NT) ? offs[4 * i] : -1;
-              const bool ok = vok && off >= 0;
-              if (!(a.dbg & 4)) ptx::cp_async16(abase + i * 512, ok ? xv + off : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
-            }
-          } else {
-            const float* wrows = a.Wcat + ((long)a.ext_atom[ext0 + c - a.kchunks] * 32 + wg) * a.ldw + v;
+          for (int i = 0; i < kRows; ++i) rows[i] = rows_t[kGatherWarps * i];
+          ptx::mbar_wait(empty_a + 8 * st_s, st_ph ^ 1);
+          const uint32_t abase = dst_thread + st_s * sbytes;
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-              ptx::cp_async16(abase + i * 512, vok ? wrows + (long)(4 * i) * a.ldw : a.X, vok ? 16u : 0u);
+          for (int i = 0; i < kRows; ++i) {
+            const bool ok = vok && rows[i] >= 0;
+            if (!(a.dbg & 4)) ptx::cp_async16(abase + i * (128 * kGatherWarps), ok ? xv + rows[i] * ldx4 : reinterpret_cast<const char*>(a.X), ok ? 16u : 0u);
           }
           // arrival on full[s] fires when all of this thread's copies above have landed: no wait here, the thread
           // goes straight on to the next chunk (gated only by that stage being free)
-          ptx::cp_async_mbar_arrive_noinc(&full[s]);
+          ptx::cp_async_mbar_arrive_noinc(full_a + 8 * st_s);
+          if (++st_s == (uint32_t)a.stages) { st_s = 0; st_ph ^= 1; }
+        }
+        for (int c = a.kchunks; c < nchunks; ++c) {
+          const float* wrows = a.Wcat + ((long)a.ext_atom[ext0 + c - a.kchunks] * 32 + wg) * a.ldw + v;
+          ptx::mbar_wait(empty_a + 8 * st_s, st_ph ^ 1);
+          const uint32_t abase = dst_thread + st_s * sbytes;
+#pragma unroll
+          for (int i = 0; i < kRows; ++i)
+            ptx::cp_async16(abase + i * (128 * kGatherWarps), vok ? wrows + (long)(kGatherWarps * i) * a.ldw : a.X, vok ? 16u : 0u);
+          ptx::cp_async_mbar_arrive_noinc(full_a + 8 * st_s);
+          if (++st_s == (uint32_t)a.stages) { st_s = 0; st_ph ^= 1; }
         }
       }
-    } else if (warp == 8) {
+    } else if (warp == kWarpTma) {
       // ================= TMA producer: H^e row block (or K-extension block), one K chunk per stage =================
-      if (lane == 0) {
-        uint32_t itc = it;
-        for (int vt = 0; vt < a.nvt; ++vt)
-          for (int c = 0; c < nchunks; ++c, ++itc) {
-            const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
-            ptx::mbar_wait(&empty[s], ph ^ 1);
-            ptx::mbar_arrive_expect_tx(&full[s], (uint32_t)bbytes);
-            const uint32_t dst = ptx::smem_u32(smem + s * sbytes + kABytes);
-            // both operand streams are stored pre-swizzled and block-contiguous: one linear bulk copy per chunk
-            const float* src = (c < a.kchunks)
-                ? a.H32t + ((long)((cell * a.NH + half) * a.kchunks + c) * a.NT) * 32 * a.ncomp
-                : a.Bext + ((long)(ext0 + c - a.kchunks) * a.NH + half) * a.NT * 32 * a.ncomp;
-            if (a.dbg & 64) { ptx::bulk_load(dst, src, (uint32_t)bbytes / 2, &full[s]); ptx::bulk_load(dst + bbytes / 2, src, (uint32_t)bbytes / 2, &full[s]); }
-            else ptx::bulk_load(dst, src, (uint32_t)bbytes, &full[s]);
+      // (the whole warp runs the loop so that every operand stays warp-uniform -- the bulk-copy and MMA instructions take
+      //  their operands from uniform registers, and per-thread values would each cost an election + broadcast sequence;
+      //  only the instructions with side effects are issued by one lane)
+      {
+        // both operand streams are stored pre-swizzled and block-contiguous: one linear bulk copy per chunk and component;
+        // PAIR: this CTA's half of the rows of every component block (NT / 2 is a multiple of 8: the swizzle phase is kept)
+        const long comp_stride = (long)a.NT * 32, chunk_stride = comp_stride * ncomp;
+        const long my_rows = PAIR ? (long)rank * (a.NT / 2) * 32 : 0;
+        const float* hsrc0 = a.H32t + (long)(cell * a.NH + half) * a.kchunks * chunk_stride + my_rows;
+        for (int j = 0; j < nsub; ++j) {
+          const float* src = hsrc0;
+          for (int c = 0; c < nchunks; ++c, src += chunk_stride) {
+            if (c == a.kchunks) src = a.Bext + ((long)ext0 * a.NH + half) * chunk_stride + my_rows;
+            const long step = c >= a.kchunks ? (long)(a.NH - 1) * chunk_stride : 0;   // extension blocks: [entry][half]
+            ptx::mbar_wait(empty_a + 8 * st_s, st_ph ^ 1);
+            const uint32_t dst = sm0 + st_s * sbytes + kABytes;
+            if (ptx::elect_one()) {
+              ptx::mbar_arrive_expect_tx(full_a + 8 * st_s, (a.dbg & 4096) ? 0u : (uint32_t)bbytes);
+              if (a.dbg & 4096) {
+              } else if (PAIR || !CPLX) {
+#pragma unroll
+                for (int comp = 0; comp < ncomp; ++comp)
+                  ptx::bulk_load(dst + comp * bbytes1, src + comp * comp_stride, (uint32_t)bbytes1, full_a + 8 * st_s);
+              } else {
+                ptx::bulk_load(dst, src, (uint32_t)bbytes, full_a + 8 * st_s);
+              }
+            }
+            src += step;
+            if (++st_s == (uint32_t)a.stages) { st_s = 0; st_ph ^= 1; }
           }
+        }
       }
       __syncwarp();
     } else {
       // ================= MMA issuer =================
-      if (lane == 0) {
-        uint32_t itc = it;
-        for (int vt = 0; vt < a.nvt; ++vt) {
-          const uint32_t buf = (sub_iter + vt) & 1, use = (sub_iter + vt) >> 1;
-          ptx::mbar_wait(&accum_empty[buf], (use & 1) ^ 1);   // buffer drained by the epilogue of two subtiles ago
+      if (PAIR && rank == 1) {
+        // rank 1 issues no MMAs: tell the leader when a stage of THIS CTA holds its operands
+        {
+          const uint32_t peer_a = ptx::map_to_rank(fpeer_a, 0);
+          for (int cnt = nchunks * nsub; cnt > 0; --cnt) {
+            ptx::mbar_wait(full_a + 8 * st_s, st_ph);
+            if (ptx::elect_one()) {
+              ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes -> tensor-core (async proxy) reads
+              // relaxed: the operands were complete in THIS CTA's shared memory when full[s] flipped (observed above), the
+              // arrival is issued after that wait, and the leader's MMA is issued after it has seen the arrival; a
+              // release at cluster scope costs a full memory barrier per chunk (measured: +0.2 ms per launch)
+              if (a.dbg & 128) ptx::mbar_arrive_cluster(peer_a + 8 * st_s); else ptx::mbar_arrive_cluster_relaxed(peer_a + 8 * st_s);
+            }
+            if (++st_s == (uint32_t)a.stages) { st_s = 0; st_ph ^= 1; }
+          }
+        }
+      } else {
+        const uint64_t adesc_c = (a.dbg & 2048) ? ptx::smem_desc_sw128(0, 16, 1024) : ptx::smem_desc(0, 4096, 512, 1);
+        const uint64_t bdesc_c = ptx::smem_desc_sw128(0, 16, 1024);
+        const uint32_t astep = (a.dbg & 2048) ? 2 : 64;
+        for (int j = 0; j < nsub; ++j) {
+          const uint32_t buf = (sub_iter + j) & 1, use = (sub_iter + j) >> 1;
+          if (PAIR) ptx::mbar_wait_cluster(acce_a + 8 * buf, (use & 1) ^ 1);
+          else ptx::mbar_wait(acce_a + 8 * buf, (use & 1) ^ 1);   // buffer drained by the epilogue of two subtiles ago
           ptx::tc_fence_after_sync();
           const uint32_t dtm = tmem_base + buf * a.acc_stride;
-          for (int c = 0; c < nchunks; ++c, ++itc) {
-            const uint32_t s = itc % a.stages, ph = (itc / a.stages) & 1;
-            ptx::mbar_wait(&full[s], ph);
-            if (!(a.dbg & 32)) ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes of the A tile -> tensor-core (async proxy) reads
+          for (int c = 0; c < nchunks; ++c) {
+            ptx::mbar_wait(full_a + 8 * st_s, st_ph);
+            if (PAIR) ptx::mbar_wait_cluster(fpeer_a + 8 * st_s, st_ph);
+            ptx::fence_proxy_async_smem();   // cp.async (generic proxy) writes of the A tile -> tensor-core (async proxy) reads
             ptx::tc_fence_after_sync();
-            const uint32_t abase = ptx::smem_u32(smem + s * sbytes), bbase = abase + kABytes;
+            // descriptors: constant fields | stage address in 16-byte units (stage bases are 1024-byte aligned)
+            //   A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
+            //     512 B apart (SBO); one K step = 8 rows = 1024 B = 64 units
+            //   B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B = 2 units per K step
+            const uint32_t a16 = (sm0 + st_s * sbytes) >> 4;
+            const uint64_t ad = adesc_c | (uint64_t)(a16 & 0x3FFF);
+            const uint64_t bd = bdesc_c | (uint64_t)((a16 + (kABytes >> 4)) & 0x3FFF);
             const int ksteps = (c == a.kchunks - 1) ? a.ksteps_last : (c >= a.kchunks ? a.ext_ksteps : kChunkK / 8);
-            for (int ks = 0; ks < ksteps; ++ks) {
-              // A (MN-major, 128B swizzle / 32B atoms): 4 blocks of 32 vectors 4096 B apart (LBO); K atoms of 4 rows
-              // 512 B apart (SBO); one K step = 8 rows = 1024 B
-              const uint64_t adesc = ptx::smem_desc(abase + ks * 1024, 4096, 512, 1);
-              // B (K-major, SW128): 8-row groups 1024 B apart (SBO); 8 tf32 = 32 B per K step inside the 128-B row
-              const uint64_t bdesc = ptx::smem_desc_sw128(bbase + ks * 32, 16, 1024);
-              if (!(a.dbg & 8)) ptx::mma_tf32_ss(dtm, adesc, bdesc, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
-              if (a.ncomp == 2) {
-                const uint64_t bdesc2 = ptx::smem_desc_sw128(bbase + bbytes1 + ks * 32, 16, 1024);
-                ptx::mma_tf32_ss(dtm + (uint32_t)a.NT, adesc, bdesc2, a.idesc, (c > 0 || ks > 0) ? 1u : 0u);
+            if (ptx::elect_one()) {
+#pragma unroll
+              for (int ks = 0; ks < kChunkK / 8; ++ks) {
+                if (ks < ksteps && !(a.dbg & 8)) {
+                  const uint32_t acc = (c | ks) != 0 ? 1u : 0u;
+                  if (PAIR) ptx::mma_tf32_ss_pair(dtm, ad + ks * astep, bd + ks * 2, a.idesc, acc);
+                  else ptx::mma_tf32_ss(dtm, ad + ks * astep, bd + ks * 2, a.idesc, acc);
+                  if (CPLX) {
+                    if (PAIR) ptx::mma_tf32_ss_pair(dtm + (uint32_t)a.NT, ad + ks * astep, bd + (bbytes1 >> 4) + ks * 2, a.idesc, acc);
+                    else ptx::mma_tf32_ss(dtm + (uint32_t)a.NT, ad + ks * astep, bd + (bbytes1 >> 4) + ks * 2, a.idesc, acc);
+                  }
+                }
               }
+              if (PAIR) ptx::mma_commit_pair(empty_a + 8 * st_s); else ptx::mma_commit(empty_a + 8 * st_s);
             }
-            ptx::mma_commit(&empty[s]);
+            __syncwarp();
+            if (++st_s == (uint32_t)a.stages) { st_s = 0; st_ph ^= 1; }
           }
-          ptx::mma_commit(&accum_full[buf]);
+          if (ptx::elect_one()) { if (PAIR) ptx::mma_commit_pair(accf_a + 8 * buf); else ptx::mma_commit(accf_a + 8 * buf); }
+          __syncwarp();
         }
       }
       __syncwarp();
     }
-    it += (uint32_t)(nchunks * a.nvt);
-    sub_iter += (uint32_t)a.nvt;
+    sub_iter += (uint32_t)nsub;
   }
-  __syncthreads();
-  if (warp == 9) ptx::tmem_dealloc(tmem_base, a.tmem_cols);
+  ptx::tc_fence_before_sync();
+  if (PAIR) ptx::cluster_sync(); else __syncthreads();   // PAIR: the peer's MMAs, commits and remote arrivals are done too
+  ptx::tc_fence_after_sync();
+  if (warp == kWarpMma) { if (PAIR) ptx::tmem_dealloc_pair(tmem_base, a.tmem_cols); else ptx::tmem_dealloc(tmem_base, a.tmem_cols); }
 }
 
 void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
@@ -341,17 +451,18 @@ void shape_for(const pawfe_ctx* c, int* NH, int* NT) {
   *NH = (c->n + maxnt - 1) / maxnt;
   int per = (c->n + *NH - 1) / *NH;
   *NT = (per + 15) / 16 * 16;
+  { const char* d = getenv("PAWFE_TC_NT"); if (d && atoi(d) >= *NT && atoi(d) <= maxnt) *NT = atoi(d); }   // timing experiments
 }
 
-size_t smem_fixed_(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + 4 * 32 * 32 * 4 + (2 * kMaxStages + 4) * 8 + 16; }
-size_t smem_fixed(int NH, int NT) { return smem_fixed_(NH, NT); }
-int stages_for(int NH, int NT, int ncomp) {
+size_t smem_fixed(int NH, int NT) { return (size_t)NH * NT * 8 + (size_t)NT * 12 + kEpiWarps * 32 * 32 * 4 + (3 * kMaxStages + 4) * 8 + 16; }
+// brows: rows of a matrix block one CTA holds per stage (NT, or NT / 2 for CTA pairs)
+int stages_for(int NH, int NT, int ncomp, int brows) {
   const size_t budget = 227 * 1024 - 1024;  // dynamic shared memory per CTA, less the alignment slack
-  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(kABytes + ncomp * NT * 128));
+  int st = (int)((budget - smem_fixed(NH, NT)) / (size_t)(kABytes + ncomp * brows * 128));
   return std::min(st, kMaxStages);
 }
-size_t smem_bytes(int NH, int NT, int ncomp) {
-  return (size_t)stages_for(NH, NT, ncomp) * (kABytes + ncomp * NT * 128) + smem_fixed(NH, NT);
+size_t smem_bytes(int NH, int NT, int ncomp, int brows) {
+  return (size_t)stages_for(NH, NT, ncomp, brows) * (kABytes + ncomp * brows * 128) + smem_fixed(NH, NT);
 }
 
 TcPlan* get_plan(pawfe_ctx* c) {
@@ -368,16 +479,10 @@ TcPlan* get_plan(pawfe_ctx* c) {
   k_retile_h32<<<8 * c->sm_count, 256, 0, c->stream>>>((const float*)c->d_H32, c->n, c->ldk, p->NH, p->NT, kchunks, ncomp, elems, p->d_H32t);
   c->launches++;
   if (cudaGetLastError() != cudaSuccess) return p;
-  // the attribute is per function, not per context: only ever raise it
-  static size_t smem_attr = 0;
-  size_t smem = smem_bytes(p->NH, p->NT, ncomp);
-  if (smem > smem_attr) {
-    if (cudaFuncSetAttribute(k_cell_tcgen05, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-      cudaGetLastError();
-      return p;
-    }
-    smem_attr = smem;
-  }
+  const void* k1 = c->cplx ? (const void*)k_cell_tcgen05<false, true> : (const void*)k_cell_tcgen05<false, false>;
+  const void* k2 = c->cplx ? (const void*)k_cell_tcgen05<true, true> : (const void*)k_cell_tcgen05<true, false>;
+  if (pawfe_ensure_smem(c, k1, smem_bytes(p->NH, p->NT, ncomp, p->NT)) != PAWFE_OK) { cudaGetLastError(); return p; }
+  if (pawfe_ensure_smem(c, k2, smem_bytes(p->NH, p->NT, ncomp, p->NT / 2)) != PAWFE_OK) { cudaGetLastError(); return p; }
   p->ok = true;
   return p;
 }
@@ -444,12 +549,16 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.nvt = (B + kTileV - 1) / kTileV;
   a.ntiles = c->ncell * a.NH;
   a.ncomp = c->cplx ? 2 : 1;
-  a.stages = stages_for(p->NH, p->NT, a.ncomp);
+  // blocks wider than one vector tile: CTA pairs (cta_group::2), both vector tiles of a pair against one load of H^e
+  const bool pair = a.nvt > 1 && c->sm_count >= 2 && !getenv("PAWFE_TC_NOPAIR");
+  const int brows = pair ? p->NT / 2 : p->NT;
+  a.stages = stages_for(p->NH, p->NT, a.ncomp, brows);
+  { const char* d = getenv("PAWFE_TC_STAGES"); if (d && atoi(d) >= 2) a.stages = std::min(a.stages, atoi(d)); }
   uint32_t cols = 32;
   while ((int)cols < a.ncomp * a.NT) cols <<= 1;
   a.acc_stride = cols;
   a.tmem_cols = 2 * cols;
-  a.idesc = ptx::idesc_tf32(kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
+  a.idesc = ptx::idesc_tf32(pair ? 2 * kTileV : kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
   a.scale_mode = 0;
   a.H32t = (ext && ext->Hstream) ? ext->Hstream : p->d_H32t; a.Bext = nullptr;
   a.ext_start = nullptr; a.ext_atom = nullptr; a.Wcat = nullptr; a.ldw = 0; a.ext_ksteps = 0;
@@ -461,8 +570,26 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
     }
   }
   { const char* d = getenv("PAWFE_TC_DBG"); a.dbg = d ? atoi(d) : 0; }
+  if (a.dbg & 2048) a.idesc = ptx::idesc_tf32(pair ? 2 * kTileV : kTileV, a.NT, 0, 0);   // timing experiment: A read as K-major (wrong results)
+  const size_t smem = smem_bytes(p->NH, p->NT, a.ncomp, brows);
+  if (pair) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * (unsigned)std::min(a.ntiles, c->sm_count / 2));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (c->cplx) CUDA_TRY(c, cudaLaunchKernelEx(&cfg, k_cell_tcgen05<true, true>, a));
+    else CUDA_TRY(c, cudaLaunchKernelEx(&cfg, k_cell_tcgen05<true, false>, a));
+    c->launches++;
+    return PAWFE_OK;
+  }
   int grid = std::min(a.ntiles, c->sm_count);
-  k_cell_tcgen05<<<grid, kThreads, smem_bytes(p->NH, p->NT, a.ncomp), c->stream>>>(a);
+  if (c->cplx) k_cell_tcgen05<false, true><<<grid, kThreads, smem, c->stream>>>(a);
+  else k_cell_tcgen05<false, false><<<grid, kThreads, smem, c->stream>>>(a);
   KERNEL_CHECK(c, "k_cell_tcgen05");
   return PAWFE_OK;
 }
