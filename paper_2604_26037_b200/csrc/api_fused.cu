@@ -31,6 +31,7 @@ struct FusedPlan {
   float* d_xlo = nullptr; size_t xlo_elems = 0;   // low parts of the input block of fused_apply_H in FP32 mode
   // second stream for work that is independent inside a step (projection || bracket prepass; mass / non-local || DMMA)
   cudaStream_t aux = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  bool no_aux = false;          // PAWFE_NO_AUX=1: everything on the context's stream (timing experiments)
   double* d_P64 = nullptr;      // [natoms][npj][ldw] FP64 projections of the residual set-up
   double* d_W64 = nullptr;      // [natoms][npj][ldw] (D - Lambda dS) P
 };
@@ -668,8 +669,8 @@ bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
 }
 
 // run `body` on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream
-#define FORK_AUX(c, p) do { CUDA_TRY(c, cudaEventRecord((p)->ev_fork, (c)->stream)); CUDA_TRY(c, cudaStreamWaitEvent((p)->aux, (p)->ev_fork, 0)); } while (0)
-#define JOIN_AUX(c, p) do { CUDA_TRY(c, cudaEventRecord((p)->ev_join, (p)->aux)); CUDA_TRY(c, cudaStreamWaitEvent((c)->stream, (p)->ev_join, 0)); } while (0)
+#define FORK_AUX(c, p) do { if ((p)->no_aux) break; CUDA_TRY(c, cudaEventRecord((p)->ev_fork, (c)->stream)); CUDA_TRY(c, cudaStreamWaitEvent((p)->aux, (p)->ev_fork, 0)); } while (0)
+#define JOIN_AUX(c, p) do { if ((p)->no_aux) break; CUDA_TRY(c, cudaEventRecord((p)->ev_join, (p)->aux)); CUDA_TRY(c, cudaStreamWaitEvent((c)->stream, (p)->ev_join, 0)); } while (0)
 struct StreamSwap {   // kernels launched while this lives go to `s`
   pawfe_ctx* c; cudaStream_t keep;
   StreamSwap(pawfe_ctx* c_, cudaStream_t s) : c(c_), keep(c_->stream) { c->stream = s; }
@@ -681,11 +682,16 @@ pawfe_status fused_prepare(pawfe_ctx* c, int B) {
   if (!p) {
     p = new FusedPlan();
     c->fused = p;
-    if (cudaStreamCreateWithFlags(&p->aux, cudaStreamNonBlocking) != cudaSuccess ||
+    // highest priority: the auxiliary kernels are short and latency-bound; their CTAs should take every slot that frees up
+    // next to the bandwidth-bound kernel of the main stream instead of queueing behind its whole grid
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if (cudaStreamCreateWithPriority(&p->aux, cudaStreamNonBlocking, getenv("PAWFE_AUX_PRIO0") ? 0 : prio_hi) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
       cudaGetLastError(); fused_invalidate(c); c->err = "fused plan: stream / event creation failed"; return PAWFE_ECUDA;
     }
+    p->no_aux = getenv("PAWFE_NO_AUX") != nullptr;
     pawfe_status st = build_plan(c, p);
     if (st != PAWFE_OK) { fused_invalidate(c); return st; }
   }
@@ -784,7 +790,7 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
     FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
     TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
     {
-      StreamSwap sw(c, p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
+      StreamSwap sw(c, p->no_aux ? c->stream : p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
       const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
       TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float>, smem));
       k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
@@ -801,7 +807,7 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   const long nquads = c->M * (ldw / 4);
   for (int th = 2; th <= m; ++th) {
     FORK_AUX(c, p);
-    { StreamSwap sw(c, p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
+    { StreamSwap sw(c, p->no_aux ? c->stream : p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
     k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
                                          ds + (size_t)(th - 1) * B, Wr, cw, (float)acs[th], (float)zzs[th]);
     KERNEL_CHECK(c, "k_prepass");

@@ -23,6 +23,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <algorithm>
+#include <vector>
 
 namespace {
 
@@ -53,12 +54,14 @@ struct TcArgs {
   // K-extension chunks (fused.h): per cell a CSR list of 32-row chunks whose A rows come from Wcat[atom]
   const int* ext_start; const int* ext_atom; const float* Wcat; long ldw; int ext_ksteps;
   const float* H32t; const float* Bext;   // pre-swizzled, block-contiguous operand streams
+  const int* order;   // tile sequence -> cell: cells in blocks of 4 x 4 x 4, so that the rows neighbouring cells share are still in L2
   int dbg;  // timing experiments only (PAWFE_TC_DBG): 1 plain stores, 2 no output, 4 no gather loads
 };
 
 struct TcPlan {
   float* d_H32t_lo = nullptr;    // low parts (value - trunc_tf32(value)) of d_H32t, FP32 mode only
   long h32t_elems = 0;
+  int* d_order = nullptr;        // cell visiting order (blocks of 4 x 4 x 4 cells)
   float* d_H32t = nullptr;       // cell matrices re-tiled for streaming: [cell][half][K chunk][NT rows][32] floats
   int NT = 0, NH = 0;
   bool ok = false;
@@ -152,8 +155,9 @@ k_cell_tcgen05(const TcArgs a) {
   uint32_t st_s = 0, st_ph = 0;   // running stage index and phase of this role's walk over the ring (same sequence in every role)
   uint32_t sub_iter = 0;          // running subtile counter: accumulator buffer = sub_iter & 1
   for (int tile = PAIR ? blockIdx.x >> 1 : blockIdx.x; tile < a.ntiles; tile += PAIR ? gridDim.x >> 1 : gridDim.x) {
-    const int cell = tile / a.NH;
-    const int half = tile - cell * a.NH;
+    const int cseq = tile / a.NH;
+    const int half = tile - cseq * a.NH;
+    const int cell = __shfl_sync(0xffffffffu, a.order[cseq], 0);
     // (values read from memory are made warp-uniform explicitly, see the note on `warp`)
     const int ext0 = __shfl_sync(0xffffffffu, a.ext_start ? a.ext_start[cell] : 0, 0);
     const int nchunks = a.kchunks + __shfl_sync(0xffffffffu, a.ext_start ? a.ext_start[cell + 1] - ext0 : 0, 0);
@@ -471,6 +475,18 @@ TcPlan* get_plan(pawfe_ctx* c) {
   c->tc_plan = p;
   shape_for(c, &p->NH, &p->NT);
   if (!c->d_H32) return p;
+  {
+    std::vector<int> order;
+    order.reserve(c->ncell);
+    const int bs = 4;
+    for (int bx = 0; bx < c->nc[0]; bx += bs)
+      for (int by = 0; by < c->nc[1]; by += bs)
+        for (int bz = 0; bz < c->nc[2]; bz += bs)
+          for (int x = bx; x < std::min(bx + bs, c->nc[0]); ++x)
+            for (int y = by; y < std::min(by + bs, c->nc[1]); ++y)
+              for (int z = bz; z < std::min(bz + bs, c->nc[2]); ++z) order.push_back((x * c->nc[1] + y) * c->nc[2] + z);
+    if (upload(c, &p->d_order, order) != PAWFE_OK) { p->d_order = nullptr; return p; }
+  }
   const int ncomp = c->cplx ? 2 : 1;
   const int kchunks = (c->ldk + kChunkK - 1) / kChunkK;
   const long elems = (long)c->ncell * p->NH * kchunks * ncomp * p->NT * 32;
@@ -521,7 +537,7 @@ pawfe_status tc_hstream_lo(pawfe_ctx* c, const float** out) {
 }
 
 void tc_invalidate(pawfe_ctx* c) {
-  if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t_lo); cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
+  if (c->tc_plan) { cudaFree(((TcPlan*)c->tc_plan)->d_H32t_lo); cudaFree(((TcPlan*)c->tc_plan)->d_order); cudaFree(((TcPlan*)c->tc_plan)->d_H32t); delete (TcPlan*)c->tc_plan; c->tc_plan = nullptr; }
 }
 
 bool tc_supported(const pawfe_ctx* c, int B) {
@@ -561,6 +577,7 @@ pawfe_status tc_cell_apply(pawfe_ctx* c, const float* X, long ldx, float* Y, lon
   a.idesc = ptx::idesc_tf32(pair ? 2 * kTileV : kTileV, a.NT, /*A MN-major*/ 1, /*B K-major*/ 0);
   a.scale_mode = 0;
   a.H32t = (ext && ext->Hstream) ? ext->Hstream : p->d_H32t; a.Bext = nullptr;
+  a.order = p->d_order;
   a.ext_start = nullptr; a.ext_atom = nullptr; a.Wcat = nullptr; a.ldw = 0; a.ext_ksteps = 0;
   if (ext) {
     a.scale_mode = ext->scale_mode;
