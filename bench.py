@@ -185,6 +185,9 @@ def run_own(args):
     dev = torch.device("cuda", local)
     prec = PREC[args.prec]
     cfg = get_config(args.config)
+    if args.block > 0:   # experiment only: another block width than BASELINE.json's (named in config.workload)
+        import dataclasses
+        cfg = dataclasses.replace(cfg, block=args.block, name=f"{cfg.name}_B{args.block}")
     sysd = make_system(cfg)
     stream = torch.cuda.current_stream()
     t_setup = time.perf_counter()
@@ -379,6 +382,7 @@ def main():
     ap.add_argument("--ring", type=int, default=8)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--resident-blocks", type=int, default=0, help="distinct vector blocks kept in HBM (0 = all)")
+    ap.add_argument("--block", type=int, default=0, help="override the config's block width B (0 = BASELINE.json's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -228,13 +228,20 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
         }
       }
     }
-#pragma unroll
-    for (int al = 0; al < NPJ; ++al) {
-      float* r = red + al * 128 + lane * 4;
-      atomicAdd(r + 0, acc[al].x); atomicAdd(r + 1, acc[al].y); atomicAdd(r + 2, acc[al].z); atomicAdd(r + 3, acc[al].w);
-    }
   }
-  __syncthreads();
+  // cross-warp sum in shared memory, one warp per round (fixed order; shared-memory float atomics are CAS loops)
+  for (int r = 0; r < 8; ++r) {
+    if (w == r && v < B) {
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) {
+        float4* q = reinterpret_cast<float4*>(red + al * 128 + lane * 4);
+        float4 t = *q;
+        t.x += acc[al].x; t.y += acc[al].y; t.z += acc[al].z; t.w += acc[al].w;
+        *q = t;
+      }
+    }
+    __syncthreads();
+  }
   for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
     const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
     if (vv < B) {
@@ -249,56 +256,54 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
 // Couplings per atom and vector (Eq. 28-29, Eq. 16):
 //   W^a = Delta^a_Sinv P1^a;  P2^a = P1^a - sum_{b in nb(a)} (G^{ab} Delta^b_Sinv) P1^b;  W2^a = D^a P2^a.
 //   mode 0: both (filter step);  mode 1: W only (recovery, S^-1approx alone);  mode 2: plain H (W = 0, W2 = D P1).
-//   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2.  grid = (natoms, ceil(B/128)), block = 128.
+//   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2.  grid = (natoms, ceil(B/32)), block = 32 * npj: one thread per
+//   (output row al, vector), so the dependent chain per thread is one dot product per neighbour instead of npj of them;
+//   P2 goes through shared memory for the last product.
 // ------------------------------------------------------------------------------------------------
+constexpr int kCoupleLanes = 32;
 template <typename T>   // float (real context) or float2 (complex context); ldp, ldw in units of T
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kCoupleLanes * PAWFE_MAX_NPJ)
 k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, const T* __restrict__ dSinv,
          const T* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
          const T* __restrict__ GD, T* __restrict__ Wcat, long ldw) {
+  __shared__ T p2s[PAWFE_MAX_NPJ][kCoupleLanes + 1];
   const int a = blockIdx.x;
-  const int v = blockIdx.y * blockDim.x + threadIdx.x;
-  if (v >= B) return;
-  T p1[PAWFE_MAX_NPJ], p2[PAWFE_MAX_NPJ];
+  const int lane = threadIdx.x % kCoupleLanes, al = threadIdx.x / kCoupleLanes;   // al < npj
+  const int v = blockIdx.y * kCoupleLanes + lane;
+  const bool ok = v < B;
+  T p1[PAWFE_MAX_NPJ];
 #pragma unroll
-  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) { p1[be] = be < npj ? P1[((long)a * npj + be) * ldp + v] : s_zero(T()); p2[be] = p1[be]; }
+  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) p1[be] = (ok && be < npj) ? P1[((long)a * npj + be) * ldp + v] : s_zero(T());
   T* Wa = Wcat + (long)a * 32 * ldw;
   if (mode != 2) {
-    const T* S = dSinv + (long)a * npj * npj;
-    for (int al = 0; al < npj; ++al) {
-      T s = s_zero(T());
+    const T* S = dSinv + ((long)a * npj + al) * npj;
+    T s = s_zero(T());
 #pragma unroll
-      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[al * npj + be], p1[be]);
-      Wa[(long)al * ldw + v] = s;
-    }
-  } else {
-    for (int al = 0; al < npj; ++al) Wa[(long)al * ldw + v] = s_zero(T());
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[be], p1[be]);
+    if (ok) Wa[(long)al * ldw + v] = s;
+  } else if (ok) {
+    Wa[(long)al * ldw + v] = s_zero(T());
   }
   if (mode == 1) return;
+  T p2 = ok ? P1[((long)a * npj + al) * ldp + v] : s_zero(T());
   if (mode == 0) {
     for (int s = nb_start[a]; s < nb_start[a + 1]; ++s) {
       const int b = nb_atom[s];
-      const T* g = GD + (long)s * npj * npj;
-      T pb[PAWFE_MAX_NPJ];
+      const T* g = GD + ((long)s * npj + al) * npj;
+      T t = s_zero(T());
 #pragma unroll
-      for (int be = 0; be < PAWFE_MAX_NPJ; ++be) pb[be] = be < npj ? P1[((long)b * npj + be) * ldp + v] : s_zero(T());
-#pragma unroll
-      for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
-        if (al < npj) {
-          T t = s_zero(T());
-#pragma unroll
-          for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(t, g[al * npj + be], pb[be]);
-          p2[al] = s_add(p2[al], s_scale(t, -1.0));
-        }
+      for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
+        if (be < npj) s_fma(t, g[be], ok ? P1[((long)b * npj + be) * ldp + v] : s_zero(T()));
+      p2 = s_add(p2, s_scale(t, -1.0));
     }
   }
-  const T* Da = D + (long)a * npj * npj;
-  for (int al = 0; al < npj; ++al) {
-    T s = s_zero(T());
+  p2s[al][lane] = p2;
+  __syncthreads();
+  const T* Da = D + ((long)a * npj + al) * npj;
+  T w2 = s_zero(T());
 #pragma unroll
-    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, Da[al * npj + be], p2[be]);
-    Wa[(long)(npj + al) * ldw + v] = s;
-  }
+  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(w2, Da[be], p2s[be][lane]);
+  if (ok) Wa[(long)(npj + al) * ldw + v] = w2;
 }
 
 // X[J][v] += scale * M_D^-1[J] * sum_al C^{e,a}[I][al] W^a[al][v] over the pairs (recovery: scale = -1).
@@ -399,16 +404,34 @@ k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, flo
 }
 
 // Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
-// by k_scatter2.  keep = 0 on Dirichlet boundary rows.
-__global__ void k_recover2(MeshDev md, long ldw, int B /*real columns*/, int cw, const float* __restrict__ RY, float* __restrict__ X,
-                           long ldx, const double* __restrict__ lamY) {
-  const long total = md.M * (long)B;
+// by k_scatter2.  keep = 0 on Dirichlet boundary rows.  VEC: 4 consecutive columns per thread (needs ldx % 4 == 0 and a
+// 16-byte aligned X; the columns beyond B of a ragged last quad are the caller's and are left untouched).
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+k_recover2(MeshDev md, long ldw, int B /*real columns*/, int cw, const float* __restrict__ RY, float* __restrict__ X,
+           long ldx, const double* __restrict__ lamY) {
+  const int nq = (B + 3) / 4;
+  const long total = md.M * (long)nq;
   for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
-    const long J = idx / B;
-    const int v = (int)(idx - J * B);
+    const long J = idx / nq;
+    const int v = (int)(idx - J * nq) * 4;
     const double keep = mdinv_row(md, J) != 0.0 ? 1.0 : 0.0;
-    const double x = (double)X[J * ldx + v];
-    X[J * ldx + v] = (float)(keep * ((double)RY[J * ldw + v] + x * lamY[v / cw]));
+    const float4 ry = *reinterpret_cast<const float4*>(RY + J * ldw + v);   // ldw % 4 == 0, pad columns readable
+    float* xp = X + J * ldx + v;
+    if (VEC && v + 3 < B) {
+      const float4 x = *reinterpret_cast<const float4*>(xp);
+      float4 o;
+      o.x = (float)(keep * ((double)ry.x + (double)x.x * lamY[v / cw]));
+      o.y = (float)(keep * ((double)ry.y + (double)x.y * lamY[(v + 1) / cw]));
+      o.z = (float)(keep * ((double)ry.z + (double)x.z * lamY[(v + 2) / cw]));
+      o.w = (float)(keep * ((double)ry.w + (double)x.w * lamY[(v + 3) / cw]));
+      *reinterpret_cast<float4*>(xp) = o;
+    } else {
+      const float r[4] = {ry.x, ry.y, ry.z, ry.w};
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (v + u < B) xp[u] = (float)(keep * ((double)r[u] + (double)xp[u] * lamY[(v + u) / cw]));
+    }
   }
 }
 
@@ -587,7 +610,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
       CASE_PC(9) CASE_PC(10) CASE_PC(11) CASE_PC(12) CASE_PC(13) CASE_PC(14) CASE_PC(15) CASE_PC(16)
 #undef CASE_PC
     }
-    k_couple<float2><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
+    k_couple<float2><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
         npj, mode, (const float2*)p->d_P1, p->ldw / 2, B, (const float2*)c->d_dSinv32, (const float2*)c->d_D32, p->d_nb_start,
         p->d_nb_atom, (const float2*)p->d_GD, (float2*)p->d_Wcat, p->ldw / 2);
     KERNEL_CHECK(c, "k_couple");
@@ -610,7 +633,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   }
 #undef LAUNCH_PROJ2
   KERNEL_CHECK(c, "k_proj2");
-  k_couple<float><<<dim3(c->natoms, ceil_div(B, 128)), 128, 0, c->stream>>>(
+  k_couple<float><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
       npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
       p->d_GD, p->d_Wcat, p->ldw);
   KERNEL_CHECK(c, "k_couple");
@@ -625,7 +648,7 @@ pawfe_status setup_nonlocal64_t(pawfe_ctx* c, FusedPlan* p, const float* X, long
   CUDA_TRY(c, cudaMemsetAsync(p->d_P64, 0, (size_t)c->natoms * NPJ * p->ldw * sizeof(double), c->stream));
   dim3 grid((unsigned)c->npairs, ceil_div(B, 64));
   {
-    const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8 + (size_t)NPJ * 64 * 8;
+    const size_t smem = (size_t)n * 8 + (size_t)NPJ * n * 8 + 8 + (size_t)NPJ * 64 * 8;
     TRY(pawfe_ensure_smem(c, (const void*)k_proj64<NPJ, float>, smem));
     k_proj64<NPJ, float><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const double*)c->d_Cd64, X, ldx, B, p->d_P64, p->ldw);
     KERNEL_CHECK(c, "k_proj64");
@@ -801,6 +824,8 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
     JOIN_AUX(c, p);
   }
   const int gs = 8 * c->sm_count;
+  int gs_pre = gs;   // timing experiments: fewer resident prepass CTAs leave room for the aux stream's projection CTAs
+  { const char* d = getenv("PAWFE_PREPASS_CPS"); if (d && atoi(d) >= 1) gs_pre = atoi(d) * c->sm_count; }
   k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
@@ -808,7 +833,7 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   for (int th = 2; th <= m; ++th) {
     FORK_AUX(c, p);
     { StreamSwap sw(c, p->no_aux ? c->stream : p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
-    k_prepass<<<gs, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
+    k_prepass<<<gs_pre, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
                                          ds + (size_t)(th - 1) * B, Wr, cw, (float)acs[th], (float)zzs[th]);
     KERNEL_CHECK(c, "k_prepass");
     JOIN_AUX(c, p);
@@ -817,7 +842,10 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----
   TRY(project_and_couple(c, p, RY, ldw, B, 1));
-  k_recover2<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
+  if ((ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0)
+    k_recover2<true><<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
+  else
+    k_recover2<false><<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
   KERNEL_CHECK(c, "k_recover2");
   if (c->npairs > 0 && c->cplx) {
     switch (c->npj) {

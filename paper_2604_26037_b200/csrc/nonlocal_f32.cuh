@@ -67,13 +67,20 @@ k_projF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
         }
       }
     }
-#pragma unroll
-    for (int al = 0; al < NPJ; ++al) {
-      float* r = red + al * 128 + lane * 4;
-      atomicAdd(r + 0, acc[al].x); atomicAdd(r + 1, acc[al].y); atomicAdd(r + 2, acc[al].z); atomicAdd(r + 3, acc[al].w);
-    }
   }
-  __syncthreads();
+  // cross-warp sum in shared memory, one warp per round (fixed order; shared-memory float atomics are CAS loops)
+  for (int r = 0; r < 8; ++r) {
+    if (w == r && v < Wr) {
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) {
+        float4* q = reinterpret_cast<float4*>(red + al * 128 + lane * 4);
+        float4 t = *q;
+        t.x += acc[al].x; t.y += acc[al].y; t.z += acc[al].z; t.w += acc[al].w;
+        *q = t;
+      }
+    }
+    __syncthreads();
+  }
   for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
     const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
     if (vv < Wr) {

@@ -68,7 +68,7 @@ k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __r
 }
 
 // P[a][al][v] += sum_I C^{e,a}[I][al] X[J(e,I)][v] in FP64.  grid = (npairs, ceil(B/64)), block = 256 (8 warps over
-// rows, lane = 2 consecutive vectors).  dynamic smem: n longs + NPJ*n doubles + NPJ*64 doubles.  P zero on entry.
+// rows, lane = 2 consecutive vectors).  dynamic smem: n longs + NPJ*n doubles + 8 bytes + NPJ*64 doubles.  P zero on entry.
 template <int NPJ, typename RX>
 __global__ void __launch_bounds__(256)
 k_proj64(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
@@ -77,7 +77,7 @@ k_proj64(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ 
   const int n = md.n, n1 = md.n1;
   long* nodeJ = reinterpret_cast<long*>(smem_raw);
   double* Cs = reinterpret_cast<double*>(nodeJ + n);   // [NPJ][n]
-  double* red = Cs + (size_t)NPJ * n;                  // [NPJ][64]
+  double* red = Cs + ((size_t)NPJ * n + ((n + (size_t)NPJ * n) & 1));   // [NPJ][64], 16-byte aligned
   const int pr = blockIdx.x, a = pair_atom[pr];
   int cx, cy, cz;
   mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
@@ -116,10 +116,20 @@ k_proj64(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ 
         }
       }
     }
-#pragma unroll
-    for (int al = 0; al < NPJ; ++al) { atomicAdd(&red[al * 64 + lane * 2], a0[al]); atomicAdd(&red[al * 64 + lane * 2 + 1], a1[al]); }
   }
-  __syncthreads();
+  // cross-warp sum in shared memory, one warp per round (fixed order; shared-memory FP64 atomics are CAS loops)
+  for (int r = 0; r < 8; ++r) {
+    if (w == r && v < B) {
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) {
+        double2* q = reinterpret_cast<double2*>(red + al * 64 + lane * 2);
+        double2 t = *q;
+        t.x += a0[al]; t.y += a1[al];
+        *q = t;
+      }
+    }
+    __syncthreads();
+  }
   for (int i = threadIdx.x; i < NPJ * 64; i += blockDim.x) {
     const int al = i >> 6, vv = blockIdx.y * 64 + (i & 63);
     if (vv < B) atomicAdd(P + ((long)a * NPJ + al) * ldp + vv, red[i]);
@@ -187,21 +197,28 @@ k_scatter64(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict
 }
 
 // Alg. 2 steps 2-3 (L260-L264) in the scaled variables:  Yt = M_D^-1 Y (FP64, in place);  Rt_Y = (zeta/e) Yt;  Rt_X = 0.
-static __global__ void k_residual_init3(MeshDev md, long ldw, int B, double* __restrict__ Y, double z_over_e,
-                                        float* __restrict__ RX, float* __restrict__ RY) {
-  const long total = md.M * ldw;
-  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
-    const long J = idx / ldw;
-    const int v = (int)(idx - J * ldw);
-    double y = 0.0;
-    if (v < B) {
-      int iz = (int)(J % md.N[2]);
-      long t = J / md.N[2];
-      int iy = (int)(t % md.N[1]), ix = (int)(t / md.N[1]);
-      y = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] * Y[idx];
-    }
-    Y[idx] = y;
-    RY[idx] = (float)(z_over_e * y);
-    RX[idx] = 0.f;
+// 4 consecutive columns per thread (ldw % 4 == 0, arrays 16-byte aligned); pad columns are written as 0.
+static __global__ void __launch_bounds__(256)
+k_residual_init3(MeshDev md, long ldw, int B, double* __restrict__ Y, double z_over_e,
+                 float* __restrict__ RX, float* __restrict__ RY) {
+  const int ldq = (int)(ldw / 4);
+  const long nquads = md.M * ldq;
+  const int N1 = md.N[1], N2 = md.N[2];
+  double2* Y2 = reinterpret_cast<double2*>(Y);
+  for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < nquads; q += (long)gridDim.x * blockDim.x) {
+    const int J = (int)(q / ldq);
+    const int v = (int)(q - (long)J * ldq) * 4;
+    const int iz = J % N2, t = J / N2;
+    const double s = md.mdinv1[0][t / N1] * md.mdinv1[1][t % N1] * md.mdinv1[2][iz];
+    double2 y0 = Y2[2 * q], y1 = Y2[2 * q + 1];
+    y0.x = v < B ? s * y0.x : 0.0;
+    y0.y = v + 1 < B ? s * y0.y : 0.0;
+    y1.x = v + 2 < B ? s * y1.x : 0.0;
+    y1.y = v + 3 < B ? s * y1.y : 0.0;
+    Y2[2 * q] = y0;
+    Y2[2 * q + 1] = y1;
+    reinterpret_cast<float4*>(RY)[q] = make_float4((float)(z_over_e * y0.x), (float)(z_over_e * y0.y),
+                                                   (float)(z_over_e * y1.x), (float)(z_over_e * y1.y));
+    reinterpret_cast<float4*>(RX)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
 }
