@@ -276,8 +276,12 @@ def run_own(args):
 
     def one(k):
         hs = host_sets[k]
-        for b in range(nblk):
-            ctx.cheb_filter_host(prec, m, b0, bW, bU, hs[b % nres].data_ptr(), lams[b % nres], B, B)
+        if nres == nblk:
+            # the pass's blocks in one call: copies of blocks k+1 / k-1 run under block k's filter
+            ctx.cheb_filter_host_set(prec, m, b0, bW, bU, [x.data_ptr() for x in hs], lams, [B] * nblk, [B] * nblk)
+        else:   # cycled resident blocks (host blocks repeat): one block per call
+            for b in range(nblk):
+                ctx.cheb_filter_host(prec, m, b0, bW, bU, hs[b % nres].data_ptr(), lams[b % nres], B, B)
 
     one(0)
     barrier()

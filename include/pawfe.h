@@ -158,6 +158,17 @@ pawfe_status pawfe_cheb_filter(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0
 pawfe_status pawfe_cheb_filter_host(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW,
                                     double bU, void* X_host, const double* lambda, long ld, int B);
 
+/* Algorithm 2 over nblk HOST vector blocks, one after the other (the blocks of one pass over the vector set, L378:
+ * "blocks of wavefunctions" are filtered independently).  Block k: X_host[k] (B[k] columns, leading dimension ld[k],
+ * element type by prec), Ritz values lambda[k] (HOST, B[k] doubles); the bounds are shared.  Same results as nblk calls
+ * of pawfe_cheb_filter_host, but pipelined over two internal device blocks: block k+1's host-to-device copy and block
+ * k-1's device-to-host copy run on the library's copy streams under block k's filter.  The host blocks should be
+ * pinned (pageable memory works but serialises the copies).  Synchronises before returning.
+ * PAWFE_EINVAL: nblk < 1, a null pointer, or arguments pawfe_cheb_filter rejects. */
+pawfe_status pawfe_cheb_filter_host_set(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                        void* const* X_host, const double* const* lambda, const long* ld,
+                                        const int* B, int nblk);
+
 /* Column 2-norms ||x_i||_2, i < B, accumulated in FP64 (L290).  X: device, element type by prec;
  * out: DEVICE, B doubles. */
 pawfe_status pawfe_col_norms(pawfe_ctx* ctx, pawfe_prec prec, const void* X, long ld, int B, double* out);

@@ -25,7 +25,7 @@ SYMBOLS = [
     "pawfe_create", "pawfe_destroy", "pawfe_last_error", "pawfe_set_stream", "pawfe_mesh_create",
     "pawfe_local_potential_gaussians", "pawfe_atoms_create", "pawfe_update_coupling", "pawfe_num_dofs",
     "pawfe_num_pairs", "pawfe_get_cell_matrix", "pawfe_get_sinv_coupling", "pawfe_apply_H", "pawfe_apply_S",
-    "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host",
+    "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read",
 ]
@@ -69,6 +69,9 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
                                       C.c_long, C.c_int, vp, C.c_size_t]
     lib.pawfe_cheb_filter_host.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, dp,
                                            C.c_long, C.c_int]
+    lib.pawfe_cheb_filter_host_set.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                               C.POINTER(C.c_void_p), C.POINTER(dp), C.POINTER(C.c_long),
+                                               C.POINTER(C.c_int), C.c_int]
     lib.pawfe_col_norms.argtypes = [vp, C.c_int, vp, C.c_long, C.c_int, vp]
     lib.pawfe_launch_count.argtypes = [vp, C.POINTER(C.c_long)]
     lib.pawfe_cell_timing.argtypes = [vp, C.c_int]
@@ -226,6 +229,17 @@ class Context:
         self._check(self.lib.pawfe_cheb_filter_host(self._h, int(prec), int(m), float(b0), float(bW), float(bU),
                                                     C.c_void_p(int(X_host_ptr)), _dptr(lam), int(ld), int(B)),
                     "pawfe_cheb_filter_host")
+
+    def cheb_filter_host_set(self, prec: int, m: int, b0: float, bW: float, bU: float, X_host_ptrs, lams, lds, Bs):
+        """Algorithm 2 over a set of HOST blocks, copies pipelined under the filters (pawfe_cheb_filter_host_set)."""
+        n = len(X_host_ptrs)
+        lams = [_f64(x) for x in lams]
+        xs = (C.c_void_p * n)(*[int(p) for p in X_host_ptrs])
+        ls = (C.POINTER(C.c_double) * n)(*[_dptr(x) for x in lams])
+        ldv = (C.c_long * n)(*[int(x) for x in lds])
+        bv = (C.c_int * n)(*[int(x) for x in Bs])
+        self._check(self.lib.pawfe_cheb_filter_host_set(self._h, int(prec), int(m), float(b0), float(bW), float(bU),
+                                                        xs, ls, ldv, bv, n), "pawfe_cheb_filter_host_set")
 
     def col_norms(self, prec: int, X, ld: int, B: int, out):
         self._check(self.lib.pawfe_col_norms(self._h, int(prec), self._ptr(X), int(ld), int(B), self._ptr(out)),

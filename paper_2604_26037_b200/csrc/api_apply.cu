@@ -80,7 +80,14 @@ pawfe_status launch_dmma(pawfe_ctx* c, const double* A, long cell_stride, const 
   if (n <= 64) return launch_dmma_mt<RX, CPLX, 2>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   if (n <= 128) return launch_dmma_mt<RX, CPLX, 4>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   if (n <= 224) return launch_dmma_mt<RX, CPLX, 7>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
-  if (n <= 352) return launch_dmma_mt<RX, CPLX, 11>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  if (n <= 352) {
+    // n = 343 (p = 6): MT = 6 is two row blocks (192 + 151 rows) at two CTAs per SM, MT = 11 one row block at one CTA per SM
+    const char* d = getenv("PAWFE_DMMA_MT");   // timing experiments
+    const int mt = d ? atoi(d) : 0;
+    if (mt == 5) return launch_dmma_mt<RX, CPLX, 5>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+    if (mt == 6) return launch_dmma_mt<RX, CPLX, 6>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+    return launch_dmma_mt<RX, CPLX, 11>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  }
   return launch_dmma_mt<RX, CPLX, 8>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
 }
 
@@ -226,9 +233,9 @@ pawfe_status pawfe_sub_SX_lambda(pawfe_ctx* c, const TX* X, long ldx, TD* Y, lon
                                  const double* neg_lam) {
   typedef typename ScalarTraits<TX>::real RX;
   constexpr int cw = ScalarTraits<TX>::cplx ? 2 : 1;
-  const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
-  TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<RX>, smem));
-  k_mass_sf<RX><<<dim3(c->ncell, ceil_div(B * cw, 32)), 256, smem, c->stream>>>(
+  const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
+  TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<RX, kMassCT>, smem));
+  k_mass_sf<RX, kMassCT><<<dim3(c->ncell, ceil_div(B * cw, kMassCT)), 256, smem, c->stream>>>(
       c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, (const RX*)X, ldx * cw, (double*)Y, ldy * cw, B * cw, neg_lam, cw);
   KERNEL_CHECK(c, "k_mass_sf");
   return pawfe_apply_nonlocal<TX, TD, TD>(c, OpData<TD>::dS(c), -1.0, X, ldx, 0, Y, ldy, 0, B, lam);

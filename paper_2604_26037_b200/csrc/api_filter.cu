@@ -242,3 +242,63 @@ extern "C" pawfe_status pawfe_cheb_filter_host(pawfe_ctx* c, pawfe_prec prec, in
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   return PAWFE_OK;
 }
+
+// Pipelined over two device blocks: H2D of block k+1 and D2H of block k-1 on the copy streams under block k's filter.
+extern "C" pawfe_status pawfe_cheb_filter_host_set(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                                   void* const* X_host, const double* const* lambda, const long* ld,
+                                                   const int* B, int nblk) {
+  if (!c) return PAWFE_EINVAL;
+  if (nblk < 1 || !X_host || !lambda || !ld || !B) { c->err = "bad block-set arguments"; return PAWFE_EINVAL; }
+  const size_t es = (prec == PAWFE_FP64 ? 8 : 4) * (c->cplx ? 2 : 1);
+  size_t blk_max = 0, need_max = 0;
+  for (int k = 0; k < nblk; ++k) {
+    TRY(check_filter(c, prec, m, b0, bW, bU, X_host[k], lambda[k], ld[k], B[k]));
+    blk_max = std::max(blk_max, (size_t)c->M * ld[k] * es);
+    need_max = std::max(need_max, filter_ws_bytes(c, prec, B[k], fused_width_ok(c, prec, B[k]) && (!c->cplx || !(ld[k] & 1))));
+  }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  auto grow = [&](void** p, size_t* have, size_t want) -> pawfe_status {
+    if (want <= *have) return PAWFE_OK;
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(*p); *p = nullptr; *have = 0;
+    char* q = nullptr; TRY(dev_alloc(c, &q, want)); *p = q; *have = want;
+    return PAWFE_OK;
+  };
+  TRY(grow(&c->d_hostblk, &c->hostblk_bytes, blk_max));
+  if (nblk > 1) TRY(grow(&c->d_hostblk2, &c->hostblk2_bytes, blk_max));
+  TRY(grow(&c->d_hostws, &c->hostws_bytes, need_max));
+  if (!c->s_h2d) {
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking));
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming));
+      CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_filt[i], cudaEventDisableTiming));
+      CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_d2h[i], cudaEventDisableTiming));
+    }
+  }
+  void* dblk[2] = {c->d_hostblk, c->d_hostblk2};
+  // the copy streams start after whatever the caller has queued on the context's stream
+  CUDA_TRY(c, cudaEventRecord(c->ev_filt[0], c->stream));
+  CUDA_TRY(c, cudaStreamWaitEvent(c->s_h2d, c->ev_filt[0], 0));
+  auto h2d = [&](int k) -> pawfe_status {
+    const int b = k & 1;
+    if (k >= 2) CUDA_TRY(c, cudaStreamWaitEvent(c->s_h2d, c->ev_d2h[b], 0));   // block k-2 has left this device block
+    CUDA_TRY(c, cudaMemcpyAsync(dblk[b], X_host[k], (size_t)c->M * ld[k] * es, cudaMemcpyHostToDevice, c->s_h2d));
+    CUDA_TRY(c, cudaEventRecord(c->ev_h2d[b], c->s_h2d));
+    return PAWFE_OK;
+  };
+  TRY(h2d(0));
+  for (int k = 0; k < nblk; ++k) {
+    const int b = k & 1;
+    if (k + 1 < nblk) TRY(h2d(k + 1));     // queued before block k's filter: runs under it
+    CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_h2d[b], 0));
+    TRY(pawfe_cheb_filter(c, prec, m, b0, bW, bU, dblk[b], lambda[k], ld[k], B[k], c->d_hostws, c->hostws_bytes));
+    CUDA_TRY(c, cudaEventRecord(c->ev_filt[b], c->stream));
+    CUDA_TRY(c, cudaStreamWaitEvent(c->s_d2h, c->ev_filt[b], 0));
+    CUDA_TRY(c, cudaMemcpyAsync(X_host[k], dblk[b], (size_t)c->M * ld[k] * es, cudaMemcpyDeviceToHost, c->s_d2h));
+    CUDA_TRY(c, cudaEventRecord(c->ev_d2h[b], c->s_d2h));
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(c->s_d2h));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return PAWFE_OK;
+}

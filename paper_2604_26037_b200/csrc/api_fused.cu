@@ -814,9 +814,9 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
     TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
     {
       StreamSwap sw(c, p->no_aux ? c->stream : p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
-      const size_t smem = (size_t)c->n * 32 * 8 + (size_t)c->n * 8;
-      TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float>, smem));
-      k_mass_sf<float><<<dim3(c->ncell, ceil_div(B, 32)), 256, smem, c->stream>>>(
+      const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
+      TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float, kMassCT>, smem));
+      k_mass_sf<float, kMassCT><<<dim3(c->ncell, ceil_div(B, kMassCT)), 256, smem, c->stream>>>(
           c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
       KERNEL_CHECK(c, "k_mass_sf");
       if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));

@@ -4,13 +4,15 @@
 //
 // One CTA = one cell x one tile of 64 real columns (64 real vectors or 32 complex ones).  The cell matrix is
 // streamed in K chunks through a 3-stage cp.async ring together with the gathered rows of X; 8 warps = 4 row
-// groups x 2 column halves, each warp owns MT x 4 DMMA tiles (8 rows x 8 columns) in registers.  Row blocks of
-// 32 MT rows are processed one after the other when n > 32 MT.
+// groups x 2 column halves, each warp owns MT x 4 DMMA tiles (8 rows x 8 columns) in registers, row tile mt*4 + rg of
+// the row block (interleaved, so the tiles of a ragged last row block spread evenly over the row groups).  Row blocks
+// of 32 MT rows are processed one after the other when n > 32 MT.  MT <= 6: two CTAs per SM (16 warps feed the DMMA pipe).
 //   complex:  Y = Hr X + Hi (iX); with interleaved (re, im) columns, iX is the pair (-im, re), so one
 //   accumulator set and two DMMAs per tile and k step do the complex product.
 #pragma once
 #include "common.h"
 #include "ptx_sm100.cuh"
+#include <type_traits>
 
 namespace dmma {
 
@@ -46,7 +48,7 @@ __device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, uint32_
 // Amat: [cell][n][n] doubles (complex: interleaved), cell_stride in scalars (0 = one shared matrix).
 // X: RX reals, ldx in reals; Y: doubles, ldy in reals; Wr = real columns (B or 2B).
 template <typename RX, bool CPLX, int MT>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, (MT <= 6 ? 2 : 1))
 k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const RX* __restrict__ X, long ldx,
             double* __restrict__ Y, long ldy, int Wr, double alpha) {
   constexpr int KC = Cfg<CPLX>::KC, strideA = Cfg<CPLX>::strideA, cw = CPLX ? 2 : 1;
@@ -136,17 +138,19 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
       ptx::cp_async_commit();
     };
 
-    issue(0);
-    if (nchunks > 1) issue(1); else ptx::cp_async_commit();
-    for (int ch = 0; ch < nchunks; ++ch) {
-      ptx::cp_async_wait<1>();
-      __syncthreads();  // chunk ch has landed for everyone; everyone is done with chunk ch - 1
-      if (ch + 2 < nchunks) issue(ch + 2); else ptx::cp_async_commit();
-      const unsigned char* st = stage0 + (size_t)(ch % kStages) * (aBytes + bBytes);
-      const double* As = reinterpret_cast<const double*>(st);
-      const RX* Bs = reinterpret_cast<const RX*>(st + aBytes);
+    // row tiles of this warp inside the cell's rows (warp-uniform; fewer than MT only in a ragged last row block)
+    int mtv = 0;
 #pragma unroll
-      for (int ks = 0; ks < KC / 4 && ntv > 0; ++ks) {
+    for (int mt = 0; mt < MT; ++mt) if (r0 + (mt * 4 + rg) * 8 < n) mtv = mt + 1;
+
+    // the DMMAs of one staged chunk.  FULLN: all four n-tiles of the warp hold columns; MTVC >= 0: the number of valid row
+    // tiles is the compile-time value (straight-line DMMAs: predicated mma.sync costs a WARPSYNC and a reload bubble per
+    // group of four, profiles/r01_ncu_small_kernels.md), -1: run-time value mtv.
+    auto mma_chunk = [&](auto fulln, auto mtvc, const double* As, const RX* Bs) {
+      constexpr bool FULLN = decltype(fulln)::value;
+      constexpr int MTVC = decltype(mtvc)::value;
+#pragma unroll
+      for (int ks = 0; ks < KC / 4; ++ks) {
         const int kk = ks * 4 + (lane & 3);
         double b[4], bi[4];
 #pragma unroll
@@ -162,30 +166,47 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
         }
 #pragma unroll
         for (int mt = 0; mt < MT; ++mt) {
-          const int row = rg * (8 * MT) + mt * 8 + (lane >> 2);
-          if (CPLX) {
-            const double2 a2 = *reinterpret_cast<const double2*>(As + row * strideA + kk * 2);
+          if (MTVC >= 0 ? mt < MTVC : mt < mtv) {             // warp-uniform
+            const int row = (mt * 4 + rg) * 8 + (lane >> 2);   // row tiles interleaved over the 4 row groups
+            if (CPLX) {
+              const double2 a2 = *reinterpret_cast<const double2*>(As + row * strideA + kk * 2);
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt)
-              if (nt < ntv) {
-                dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.x, b[nt]);
-                dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.y, bi[nt]);
-              }
-          } else {
-            const double a1 = As[row * strideA + kk];
+              for (int nt = 0; nt < 4; ++nt)
+                if (FULLN || nt < ntv) {
+                  dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.x, b[nt]);
+                  dmma884(acc[mt][nt][0], acc[mt][nt][1], a2.y, bi[nt]);
+                }
+            } else {
+              const double a1 = As[row * strideA + kk];
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt)
-              if (nt < ntv) dmma884(acc[mt][nt][0], acc[mt][nt][1], a1, b[nt]);
+              for (int nt = 0; nt < 4; ++nt)
+                if (FULLN || nt < ntv) dmma884(acc[mt][nt][0], acc[mt][nt][1], a1, b[nt]);
+            }
           }
         }
       }
+    };
+
+    issue(0);
+    if (nchunks > 1) issue(1); else ptx::cp_async_commit();
+    for (int ch = 0; ch < nchunks; ++ch) {
+      ptx::cp_async_wait<1>();
+      __syncthreads();  // chunk ch has landed for everyone; everyone is done with chunk ch - 1
+      if (ch + 2 < nchunks) issue(ch + 2); else ptx::cp_async_commit();
+      const unsigned char* st = stage0 + (size_t)(ch % kStages) * (aBytes + bBytes);
+      const double* As = reinterpret_cast<const double*>(st);
+      const RX* Bs = reinterpret_cast<const RX*>(st + aBytes);
+      if (ntv == 4 && mtv == MT) mma_chunk(std::true_type(), std::integral_constant<int, MT>(), As, Bs);
+      else if (ntv == 4 && mtv == MT - 1) mma_chunk(std::true_type(), std::integral_constant<int, MT - 1>(), As, Bs);
+      else if (ntv == 4) mma_chunk(std::true_type(), std::integral_constant<int, -1>(), As, Bs);
+      else if (ntv > 0) mma_chunk(std::false_type(), std::integral_constant<int, -1>(), As, Bs);
     }
     ptx::cp_async_wait<0>();
     __syncthreads();  // ring free for the next row block
     // assembly (step iv): atomic adds of the 8 x 8 tiles
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
-      const int I = r0 + rg * (8 * MT) + mt * 8 + (lane >> 2);
+      const int I = r0 + (mt * 4 + rg) * 8 + (lane >> 2);
       const long J = I < n ? nodeJ[I] : -1;
       if (J < 0) continue;
 #pragma unroll

@@ -192,6 +192,10 @@ struct pawfe_ctx {
   void* d_hostblk = nullptr; size_t hostblk_bytes = 0;
   void* d_hostws = nullptr;  size_t hostws_bytes = 0;
   void* h_stage = nullptr;   size_t stage_bytes = 0;
+  // pipelined host-buffer filter over a block set (pawfe_cheb_filter_host_set): second device block, copy streams, events
+  void* d_hostblk2 = nullptr; size_t hostblk2_bytes = 0;
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_filt[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
 };
 
 #define CUDA_TRY(ctx, call)                                                                   \

@@ -91,7 +91,14 @@ extern "C" pawfe_status pawfe_destroy(pawfe_ctx* c) {
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   cudaFree(c->d_scal);
   for (int i = 0; i < pawfe_ctx::kScalSlots; ++i) if (c->scal_ev[i]) cudaEventDestroy(c->scal_ev[i]);
-  cudaFree(c->d_hostblk); cudaFree(c->d_hostws);
+  cudaFree(c->d_hostblk); cudaFree(c->d_hostws); cudaFree(c->d_hostblk2);
+  if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
+  if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
+  for (int i = 0; i < 2; ++i) {
+    if (c->ev_h2d[i]) cudaEventDestroy(c->ev_h2d[i]);
+    if (c->ev_filt[i]) cudaEventDestroy(c->ev_filt[i]);
+    if (c->ev_d2h[i]) cudaEventDestroy(c->ev_d2h[i]);
+  }
   if (c->h_stage) cudaFreeHost(c->h_stage);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;

@@ -8,18 +8,21 @@
 #pragma once
 #include "common.h"
 
-// Y[J][v] += coef[v / cw] * (M^e X_e)[I][v] over all cells (coef = null: +1; cw = 2: interleaved complex columns).  grid = (ncell, ceil(W/32)), block = 256.
-//   dynamic smem: n * 32 doubles + n longs.  M1: [n1][n1] doubles (device).
-template <typename RX>
-__global__ void __launch_bounds__(256)
+// Y[J][v] += coef[v / cw] * (M^e X_e)[I][v] over all cells (coef = null: +1; cw = 2: interleaved complex columns).
+//   grid = (ncell, ceil(W/CT)), block = 256.  dynamic smem: n * CT doubles + n longs.  M1: [n1][n1] doubles (device).
+//   CT = 16 columns per CTA: 47 KB of shared memory, so four CTAs per SM overlap their gather / sweep / reduction phases
+//   (the kernel is latency-bound: ncu, profiles/r01_ncu_small_kernels.md).
+constexpr int kMassCT = 16;
+template <typename RX, int CT>
+__global__ void __launch_bounds__(256, 4)
 k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __restrict__ X, long ldx,
           double* __restrict__ Y, long ldy, int W, const double* __restrict__ coef, int cw = 1) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = md.n, n1 = md.n1, n2 = n1 * n1;
-  double* U = reinterpret_cast<double*>(smem_raw);    // [n][32]
-  long* nodeJ = reinterpret_cast<long*>(U + (size_t)n * 32);
+  double* U = reinterpret_cast<double*>(smem_raw);    // [n][CT]
+  long* nodeJ = reinterpret_cast<long*>(U + (size_t)n * CT);
   __shared__ double m1s[PAWFE_MAX_N1 * PAWFE_MAX_N1];
-  const int v0 = blockIdx.y * 32;
+  const int v0 = blockIdx.y * CT;
   int cx, cy, cz;
   mesh_cell_coords(md, blockIdx.x, &cx, &cy, &cz);
   for (int I = threadIdx.x; I < n; I += blockDim.x) {
@@ -30,8 +33,9 @@ k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __r
   }
   for (int i = threadIdx.x; i < n2; i += blockDim.x) m1s[i] = M1[i];
   __syncthreads();
-  for (int i = threadIdx.x; i < n * 32; i += blockDim.x) {
-    const int I = i >> 5, col = i & 31;
+#pragma unroll 4
+  for (int i = threadIdx.x; i < n * CT; i += blockDim.x) {
+    const int I = i / CT, col = i % CT;
     const long J = nodeJ[I];
     U[i] = (J >= 0 && v0 + col < W) ? (double)X[J * ldx + v0 + col] : 0.0;
   }
@@ -39,8 +43,8 @@ k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __r
   // three sweeps: direction d has stride n1^(2-d); a work item is one line (n1 values) of one column
   for (int d = 2; d >= 0; --d) {
     const int stride = d == 2 ? 1 : (d == 1 ? n1 : n2);
-    for (int i = threadIdx.x; i < n2 * 32; i += blockDim.x) {
-      const int col = i & 31, line = i >> 5;
+    for (int i = threadIdx.x; i < n2 * CT; i += blockDim.x) {
+      const int col = i % CT, line = i / CT;
       const int q0 = line / n1, q1 = line % n1;   // the two fixed indices
       int base;
       if (d == 2) base = (q0 * n1 + q1) * n1;          // (a, b, .)
@@ -48,20 +52,20 @@ k_mass_sf(MeshDev md, const double* __restrict__ M1, double scale, const RX* __r
       else base = q0 * n1 + q1;                        // (., b, c)
       double t[PAWFE_MAX_N1];
 #pragma unroll
-      for (int k = 0; k < PAWFE_MAX_N1; ++k) t[k] = k < n1 ? U[(base + k * stride) * 32 + col] : 0.0;
+      for (int k = 0; k < PAWFE_MAX_N1; ++k) t[k] = k < n1 ? U[(base + k * stride) * CT + col] : 0.0;
 #pragma unroll
       for (int r = 0; r < PAWFE_MAX_N1; ++r)
         if (r < n1) {
           double s = 0.0;
 #pragma unroll
           for (int k = 0; k < PAWFE_MAX_N1; ++k) if (k < n1) s = fma(m1s[r * n1 + k], t[k], s);
-          U[(base + r * stride) * 32 + col] = s;
+          U[(base + r * stride) * CT + col] = s;
         }
     }
     __syncthreads();
   }
-  for (int i = threadIdx.x; i < n * 32; i += blockDim.x) {
-    const int I = i >> 5, col = i & 31;
+  for (int i = threadIdx.x; i < n * CT; i += blockDim.x) {
+    const int I = i / CT, col = i % CT;
     const long J = nodeJ[I];
     if (J >= 0 && v0 + col < W) atomicAdd(Y + J * ldy + v0 + col, (coef ? coef[(v0 + col) / cw] : 1.0) * scale * U[i]);
   }
