@@ -88,24 +88,31 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
 #pragma unroll
       for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
+    constexpr int RPP = kThreads / KC, NJ = RB / RPP;   // rows per sweep of the CTA, sweeps per chunk
+    static_assert(RB % RPP == 0, "row block must be a multiple of the rows per sweep");
+    const int ak = threadIdx.x % KC, arow0 = threadIdx.x / KC;
+    const double* srcA = A + ((long)(r0 + arow0) * n + ak) * cw;
+    const uint32_t dstA = (uint32_t)(arow0 * strideA + ak * cw) * 8;
+    const int nrow_valid = n - r0 - arow0;              // row arow0 + RPP j of the block exists iff RPP j < nrow_valid
+    const long rstep = (long)RPP * n * cw;
+
     auto issue = [&](int ch) {
       unsigned char* st = stage0 + (size_t)(ch % kStages) * (aBytes + bBytes);
       const uint32_t abase = ptx::smem_u32(st), bbase = abase + (uint32_t)aBytes;
       const int k0 = ch * KC;
-      if (CPLX) {
-        // matrix rows: KC double2 per row, 16-byte copies
-        for (int i = threadIdx.x; i < RB * KC; i += kThreads) {
-          const int row = i / KC, k = i % KC;
-          const bool ok = (r0 + row < n) && (k0 + k < n);
-          const double* src = ok ? A + ((long)(r0 + row) * n + k0 + k) * 2 : A;
-          ptx::cp_async16(abase + (uint32_t)(row * strideA + k * 2) * 8, src, ok ? 16u : 0u);
-        }
-      } else {
-        for (int i = threadIdx.x; i < RB * KC; i += kThreads) {
-          const int row = i / KC, k = i % KC;
-          const bool ok = (r0 + row < n) && (k0 + k < n);
-          const double* src = ok ? A + (long)(r0 + row) * n + k0 + k : A;
-          cp_async8(abase + (uint32_t)(row * strideA + k) * 8, src, ok ? 8u : 0u);
+      // matrix rows: thread t copies element ak = t % KC of the rows arow0 + RPP j (RPP = kThreads / KC rows per sweep);
+      // source and destination advance by constants, so a copy costs a pointer add and a select (the index arithmetic of
+      // the generic loop took ~45% of the warps' time: profiles/r01_ncu_small_kernels.md)
+      {
+        const bool kok = k0 + ak < n;
+        const double* sj = srcA + (long)k0 * cw;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+          const bool ok = kok && (RPP * j < nrow_valid);
+          const uint32_t dst = abase + dstA + (uint32_t)(j * RPP * strideA * 8);
+          if (CPLX) ptx::cp_async16(dst, ok ? sj : A, ok ? 16u : 0u);
+          else cp_async8(dst, ok ? sj : A, ok ? 8u : 0u);
+          sj += rstep;
         }
       }
       // gathered X rows: KC rows x 64 reals

@@ -307,3 +307,38 @@ def test_filter_complex_odd_width_generic_sequence():
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
     assert _relerr(_to_host(Xd, True), want) < 5e-2
+
+
+@pytest.mark.parametrize("name,prec", [("cfg1_twin", "fp32"), ("cfg3_twin", "tf32"), ("cfg0", "fp64")])
+def test_filter_host_block_set(name, prec):
+    """pawfe_cheb_filter_host_set: three pinned HOST blocks of different widths (the third reuses the first device
+    block of the two-block pipeline) against the oracle's filter of each block; also equal to the device-block call."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import PREC
+    cfg, sysd, ops, ctx = _setup(name)
+    m = 4
+    widths = [cfg.block, max(2, cfg.block // 2), cfg.block - 2]
+    Xs, lams, wants = [], [], []
+    for k, B in enumerate(widths):
+        X0 = random_block(cfg, B, stream=40 + k) * ops.mask[:, None]
+        X = chfsi.s_orthonormalise(ops.apply_S, X0)
+        X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+        Xs.append(X); lams.append(lam)
+    b0 = min(l[0] for l in lams) - 0.1
+    bW = max(l[-1] for l in lams) + 0.05
+    bU = _bounds(ops, lams[0])[2]
+    for X, lam in zip(Xs, lams):
+        wants.append(chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU))
+    host = [_to_dev(X, prec, cfg.complex).cpu().pin_memory() for X in Xs]
+    dev = [h.cuda() for h in host]
+    ctx.cheb_filter_host_set(PREC[prec], m, b0, bW, bU, [h.data_ptr() for h in host], lams, widths, widths)
+    tol = {"fp64": 1e-10, "fp32": 5e-4, "tf32": 5e-2}[prec]
+    for k, B in enumerate(widths):
+        got = _to_host(host[k], cfg.complex)
+        assert _relerr(got, wants[k]) < tol, (name, prec, k, _relerr(got, wants[k]))
+        nbytes = ctx.filter_workspace(PREC[prec], B)
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        ctx.cheb_filter(PREC[prec], m, b0, bW, bU, dev[k], lams[k], B, B, ws, nbytes)
+        torch.cuda.synchronize()
+        # same kernels on the same data: equal up to the order of the FP32 assembly reductions (DESIGN.md R20)
+        assert _relerr(_to_host(dev[k], cfg.complex), got) < (1e-13 if prec == "fp64" else 1e-5)
