@@ -21,6 +21,9 @@ struct FusedPlan {
   int* d_nb_start = nullptr;    // [natoms + 1]
   int* d_nb_atom = nullptr;     // [nnb]
   float* d_GD = nullptr;        // [nnb][npj][npj]:  G^{ab} Delta^b_Sinv
+  int* d_cps = nullptr;         // [ncell + 1] cell -> its (cell, atom) pairs
+  int* d_cpi = nullptr;         // [npairs] pair indices by cell
+  bool ppfuse = false;          // PAWFE_PPFUSE=1: bracket and projection in one sweep (k_prepass_proj; slower so far)
   int ext_ksteps = 4;
   // scratch for block width <= Bcap
   int Bcap = 0; long ldw = 0;
@@ -403,6 +406,127 @@ k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, flo
   }
 }
 
+// Bracket of Alg. 2 step 4 (as k_prepass) and the projection P1 = C^T Rt_Y (as k_proj2) in ONE sweep over Rt_Y: a CTA is a
+// cell x 128 columns; it reads the cell's rows once, writes the bracket for the nodes the cell owns (every node has exactly
+// one owner cell) and accumulates the projection of the cell's first (cell, atom) pair on the rows it already holds;
+// further pairs of the cell re-read the rows (L1 / L2 hits).  The streaming part leaves the issue slots to the FMAs of
+// the projection, which as a kernel of its own was issue / latency-bound (profiles/r01_ncu_small_kernels.md).
+// Opt-in (PAWFE_PPFUSE=1): parity-green, but at 2 CTAs x 256 threads per SM and two rows in flight per thread it moves
+// 4.2 GB in 1.02 ms (4.1 TB/s) against 0.53 + 0.29 ms for k_prepass + k_proj2, so the separate kernels stay the default.
+//   grid = (ncell, ceil(ldw/128)), block = 256.  dynamic smem: n longs + NPJ*n floats + NPJ*128 floats + n bytes.
+//   P zero on entry.  Real contexts.  ldw % 4 == 0; P rows have ldp >= ldw.
+template <int NPJ>
+__global__ void __launch_bounds__(256, 2)
+k_prepass_proj(MeshDev md, const int* __restrict__ cps, const int* __restrict__ cpi, const int* __restrict__ pair_atom,
+               const float* __restrict__ Cd, const float* __restrict__ RY, float* __restrict__ RX,
+               const double* __restrict__ Yt, long ldw, int B, const double* __restrict__ aLamY, float ac, float zz1,
+               float* __restrict__ P, long ldp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = md.n, n1 = md.n1, pp = md.p;
+  long* nodeJ = reinterpret_cast<long*>(smem_raw);                       // row index (always valid)
+  float* Cs = reinterpret_cast<float*>(nodeJ + (n + 1) / 2 * 2);         // [NPJ][n]
+  float* red = Cs + ((size_t)NPJ * n + 3) / 4 * 4;                       // [NPJ][128]
+  unsigned char* flag = reinterpret_cast<unsigned char*>(red + NPJ * 128);   // bit 0: owned by this cell, bit 1: masked
+  const int e = blockIdx.x;
+  const int q0 = cps[e], nq = cps[e + 1] - q0;
+  int cx, cy, cz;
+  mesh_cell_coords(md, e, &cx, &cy, &cz);
+  for (int I = threadIdx.x; I < n; I += blockDim.x) {
+    int c = I % n1, b = (I / n1) % n1, a = I / (n1 * n1), ix, iy, iz;
+    nodeJ[I] = mesh_node(md, cx, cy, cz, a, b, c, &ix, &iy, &iz);
+    const bool own = (a < pp || (!md.periodic && cx == md.nc[0] - 1)) && (b < pp || (!md.periodic && cy == md.nc[1] - 1)) &&
+                     (c < pp || (!md.periodic && cz == md.nc[2] - 1));
+    const bool masked = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0;
+    flag[I] = (own ? 1 : 0) | (masked ? 2 : 0);
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int v = blockIdx.y * 128 + lane * 4;
+  const bool vok = v < ldw;
+  double l0 = 0, l1 = 0, l2 = 0, l3 = 0;
+  if (v < B) l0 = aLamY[v];
+  if (v + 1 < B) l1 = aLamY[v + 1];
+  if (v + 2 < B) l2 = aLamY[v + 2];
+  if (v + 3 < B) l3 = aLamY[v + 3];
+  for (int q = 0; q < (nq > 0 ? nq : 1); ++q) {
+    const int pr = nq > 0 ? cpi[q0 + q] : -1;
+    __syncthreads();   // nodeJ / flag written (q = 0); everyone is done with Cs and red of the previous pair
+    if (pr >= 0) {
+      for (int i = threadIdx.x; i < NPJ * n; i += blockDim.x) Cs[i] = Cd[(long)pr * NPJ * n + i];
+      for (int i = threadIdx.x; i < NPJ * 128; i += blockDim.x) red[i] = 0.f;
+    }
+    __syncthreads();
+    float4 acc[NPJ];
+#pragma unroll
+    for (int al = 0; al < NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (vok) {
+      // rows w, w + 8, ...; two rows in flight per thread
+      for (int I0 = w; I0 < n; I0 += 16) {
+        float4 ry[2], rx[2];
+        double2 ya[2], yb[2];
+        int fl[2];
+        long off[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int I = I0 + 8 * u;
+          fl[u] = I < n ? flag[I] : 2;
+          off[u] = I < n ? nodeJ[I] * ldw + v : 0;
+          const bool brk = I < n && q == 0 && (fl[u] & 1);
+          const bool prj = pr >= 0 && !(fl[u] & 2);
+          fl[u] = (brk ? 1 : 0) | (prj ? 2 : 0);
+          ry[u] = (brk || prj) ? __ldg(reinterpret_cast<const float4*>(RY + off[u])) : make_float4(0.f, 0.f, 0.f, 0.f);
+          if (brk) {
+            rx[u] = *reinterpret_cast<const float4*>(RX + off[u]);
+            ya[u] = __ldg(reinterpret_cast<const double2*>(Yt + off[u]));
+            yb[u] = __ldg(reinterpret_cast<const double2*>(Yt + off[u] + 2));
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          if (fl[u] & 1) {
+            float4 o;
+            o.x = (float)((double)(-ac * ry[u].x - zz1 * rx[u].x) + ya[u].x * l0);
+            o.y = (float)((double)(-ac * ry[u].y - zz1 * rx[u].y) + ya[u].y * l1);
+            o.z = (float)((double)(-ac * ry[u].z - zz1 * rx[u].z) + yb[u].x * l2);
+            o.w = (float)((double)(-ac * ry[u].w - zz1 * rx[u].w) + yb[u].y * l3);
+            *reinterpret_cast<float4*>(RX + off[u]) = o;
+          }
+          if (fl[u] & 2) {
+            const int I = I0 + 8 * u;
+#pragma unroll
+            for (int al = 0; al < NPJ; ++al) {
+              const float cv = Cs[al * n + I];
+              acc[al].x = fmaf(cv, ry[u].x, acc[al].x); acc[al].y = fmaf(cv, ry[u].y, acc[al].y);
+              acc[al].z = fmaf(cv, ry[u].z, acc[al].z); acc[al].w = fmaf(cv, ry[u].w, acc[al].w);
+            }
+          }
+        }
+      }
+    }
+    if (pr < 0) break;   // uniform: a cell without pairs only writes the bracket
+    for (int r = 0; r < 8; ++r) {   // ordered cross-warp sum
+      if (w == r && vok) {
+#pragma unroll
+        for (int al = 0; al < NPJ; ++al) {
+          float4* qd = reinterpret_cast<float4*>(red + al * 128 + lane * 4);
+          float4 t = *qd;
+          t.x += acc[al].x; t.y += acc[al].y; t.z += acc[al].z; t.w += acc[al].w;
+          *qd = t;
+        }
+      }
+      __syncthreads();
+    }
+    const int a = pair_atom[pr];
+    for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
+      const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
+      if (vv < ldw) {
+        const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
+        float* dst = P + ((long)a * NPJ + al) * ldp + vv;
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
+      }
+    }
+  }
+}
+
 // Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
 // by k_scatter2.  keep = 0 on Dirichlet boundary rows.  VEC: 4 consecutive columns per thread (needs ldx % 4 == 0 and a
 // 16-byte aligned X; the columns beyond B of a ragged last quad are the caller's and are left untouched).
@@ -438,7 +562,7 @@ k_recover2(MeshDev md, long ldw, int B /*real columns*/, int cw, const float* __
 void free_plan(FusedPlan* p) {
   if (!p) return;
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
-  cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD);
+  cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD); cudaFree(p->d_cps); cudaFree(p->d_cpi);
   cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
   cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
   if (p->aux) cudaStreamDestroy(p->aux);
@@ -499,10 +623,11 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   p->ext_ksteps = (2 * npj + 7) / 8;
   if (p->nchunks == 0) { p->ok = true; return PAWFE_OK; }
 
-  int *d_ec = nullptr, *d_cps = nullptr, *d_cpi = nullptr;
+  int* d_ec = nullptr;
+  int *&d_cps = p->d_cps, *&d_cpi = p->d_cpi;   // kept: the fused prepass + projection kernel walks the cells' pairs
   double* d_G = nullptr;
   pawfe_status st = PAWFE_OK;
-  auto cleanup = [&]() { cudaFree(d_ec); cudaFree(d_cps); cudaFree(d_cpi); cudaFree(d_G); };
+  auto cleanup = [&]() { cudaFree(d_ec); cudaFree(d_G); };
 #define TRYP(xx) do { st = (xx); if (st != PAWFE_OK) { cleanup(); return st; } } while (0)
   TRYP(upload(c, &p->d_ext_start, es)); TRYP(upload(c, &p->d_ext_atom, ea)); TRYP(upload(c, &d_ec, ec));
   TRYP(upload(c, &d_cps, cps)); TRYP(upload(c, &d_cpi, cpi));
@@ -599,9 +724,16 @@ pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, 
 }
 
 // X: the block as floats (complex: interleaved), ldx in floats; B vectors.
-pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
+pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode, bool projected = false) {
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
+  if (projected) {   // P1 already holds C^T X (k_prepass_proj): couplings only
+    k_couple<float><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
+        npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
+        p->d_GD, p->d_Wcat, p->ldw);
+    KERNEL_CHECK(c, "k_couple");
+    return PAWFE_OK;
+  }
   CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
   if (c->cplx) {
     switch (npj) {
@@ -715,6 +847,7 @@ pawfe_status fused_prepare(pawfe_ctx* c, int B) {
       cudaGetLastError(); fused_invalidate(c); c->err = "fused plan: stream / event creation failed"; return PAWFE_ECUDA;
     }
     p->no_aux = getenv("PAWFE_NO_AUX") != nullptr;
+    p->ppfuse = getenv("PAWFE_PPFUSE") != nullptr;
     pawfe_status st = build_plan(c, p);
     if (st != PAWFE_OK) { fused_invalidate(c); return st; }
   }
@@ -784,6 +917,30 @@ static pawfe_status scatter_cplx(pawfe_ctx* c, FusedPlan* p, float* X, long ldx,
   return PAWFE_OK;
 }
 
+pawfe_status launch_prepass_proj(pawfe_ctx* c, FusedPlan* p, const float* RY, float* RX, const double* Yt, long ldw, int B,
+                                 const double* aLamY, float ac, float zz1) {
+  const int n = c->n, npj = c->npj;
+  const size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4 + (size_t)(n + 15) / 16 * 16;
+  dim3 grid((unsigned)c->ncell, ceil_div((int)ldw, 128));
+#define LAUNCH_PP(NPJ)                                                                                               \
+  do {                                                                                                               \
+    TRY(pawfe_ensure_smem(c, (const void*)k_prepass_proj<NPJ>, smem));                                               \
+    k_prepass_proj<NPJ><<<grid, 256, smem, c->stream>>>(c->md, p->d_cps, p->d_cpi, c->d_pair_atom, (const float*)c->d_Cd32, RY, RX, \
+                                                        Yt, ldw, B, aLamY, ac, zz1, p->d_P1, p->ldw);                  \
+  } while (0)
+  switch (npj) {
+    case 1: LAUNCH_PP(1); break;   case 2: LAUNCH_PP(2); break;   case 3: LAUNCH_PP(3); break;
+    case 4: LAUNCH_PP(4); break;   case 5: LAUNCH_PP(5); break;   case 6: LAUNCH_PP(6); break;
+    case 7: LAUNCH_PP(7); break;   case 8: LAUNCH_PP(8); break;   case 9: LAUNCH_PP(9); break;
+    case 10: LAUNCH_PP(10); break; case 11: LAUNCH_PP(11); break; case 12: LAUNCH_PP(12); break;
+    case 13: LAUNCH_PP(13); break; case 14: LAUNCH_PP(14); break; case 15: LAUNCH_PP(15); break;
+    default: LAUNCH_PP(16); break;
+  }
+#undef LAUNCH_PP
+  KERNEL_CHECK(c, "k_prepass_proj");
+  return PAWFE_OK;
+}
+
 // X: the block in the context's FP32 storage scalar (float, or float2 interleaved), ld and B in those scalars.  Inside, every
 // array is a real block of Wr = B * cw columns (cw = 2 for complex contexts) with leading dimension ldw = roundup4(Wr).
 pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds, const double* as, const double* acs,
@@ -830,7 +987,16 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   KERNEL_CHECK(c, "k_residual_init3");
   // ---- step 4 ----
   const long nquads = c->M * (ldw / 4);
+  const bool ppfuse = !c->cplx && c->npairs > 0 && p->d_cps && p->ppfuse;
   for (int th = 2; th <= m; ++th) {
+    if (ppfuse) {   // bracket and projection in one sweep over Rt_Y, then the couplings
+      CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * c->npj * p->ldw * sizeof(float), c->stream));
+      TRY(launch_prepass_proj(c, p, RY, RX, Yt, ldw, Wr, ds + (size_t)(th - 1) * B, (float)acs[th], (float)zzs[th]));
+      TRY(project_and_couple(c, p, RY, ldw, B, 0, true));
+      TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, XLO));
+      std::swap(RX, RY);
+      continue;
+    }
     FORK_AUX(c, p);
     { StreamSwap sw(c, p->no_aux ? c->stream : p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
     k_prepass<<<gs_pre, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
