@@ -368,3 +368,110 @@ def test_filter_fused_prepass_projection_variant(name, monkeypatch):
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
     assert _relerr(_to_host(Xd, False), want) < 5e-2
+
+
+# ---- degenerate and extreme cases --------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("name,prec", [("cfg1_twin", "tf32"), ("cfg1_twin", "fp64"), ("cfg3_twin", "tf32"), ("cfg4_twin", "fp32")])
+def test_filter_degree_one(name, prec):
+    """m = 1 (reading R22): the step loop is empty, Psi_f = S^-1approx R_1 + X Lambda_1 from the FP64 residual alone."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import PREC
+    cfg, sysd, ops, ctx = _setup(name)
+    B = cfg.block
+    X0 = random_block(cfg, B, stream=51) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, 1, b0, bW, bU)
+    Xd = _to_dev(X, prec, cfg.complex)
+    nbytes = ctx.filter_workspace(PREC[prec], B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(PREC[prec], 1, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, cfg.complex), want) < {"fp64": 1e-10, "fp32": 5e-5, "tf32": 5e-5}[prec]
+
+
+@pytest.mark.parametrize("name", ["cfg1_twin", "cfg4_twin"])
+def test_single_vector_block(name):
+    """B = 1: one column (workspace rows padded to 4, one partially filled vector tile)."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import FP32, TF32
+    cfg, sysd, ops, ctx = _setup(name)
+    X = random_block(cfg, 1, stream=52) * ops.mask[:, None]
+    Xd = _to_dev(X, "fp32", False)
+    Yd = torch.empty_like(Xd)
+    ctx.apply_H(FP32, Xd, Yd, 1, 1)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Yd, False), ops.apply_H(X) * ops.mask[:, None]) < TOL["fp32"]
+    Xs = chfsi.s_orthonormalise(ops.apply_S, X)
+    Xs, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, Xs)
+    b0, bW, bU = _bounds(ops, lam)
+    m = 4
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, Xs, lam, m, b0, bW, bU)
+    Xd = _to_dev(Xs, "tf32", False)
+    nbytes = ctx.filter_workspace(TF32, 1)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, 1, 1, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, False), want) < 5e-2
+
+
+def test_maximum_block_width():
+    """B = 512, the widest block the library accepts (four vector tiles per cell): H X in every mode, one filter call."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import PREC, TF32
+    cfg, sysd, ops, ctx = _setup("cfg1_twin")
+    B = 512
+    X = random_block(cfg, B, stream=53) * ops.mask[:, None]
+    want = ops.apply_H(X) * ops.mask[:, None]
+    for prec in ("fp64", "fp32", "tf32"):
+        Xd = _to_dev(X, prec, False)
+        Yd = torch.full_like(Xd, float("nan"))
+        ctx.apply_H(PREC[prec], Xd, Yd, B, B)
+        torch.cuda.synchronize()
+        assert _relerr(_to_host(Yd, False), want) < TOL[prec], prec
+    Xs = chfsi.s_orthonormalise(ops.apply_S, X)
+    Xs, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, Xs)
+    b0, bW, bU = _bounds(ops, lam)
+    m = 3
+    wantf = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, Xs, lam, m, b0, bW, bU)
+    Xd = _to_dev(Xs, "tf32", False)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, False), wantf) < 5e-2
+
+
+def test_error_behaviour():
+    """Every call returns a status (include/pawfe.h): bad arguments are PAWFE_EINVAL, calls before set-up PAWFE_ESTATE; the
+    block is left untouched."""
+    from paper_2604_26037_b200 import Context, PawfeError, PERIODIC, TF32
+    cfg, sysd, ops, ctx = _setup("cfg1_twin")
+    B = 8
+    X = _to_dev(random_block(cfg, B, stream=54), "tf32", False)
+    X0 = X.clone()
+    lam = np.linspace(-1.0, 0.0, B)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.cheb_filter(TF32, 4, -2.0, 1.0, 0.5, X, lam, B, B, ws, nbytes)          # bW >= bU
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.cheb_filter(TF32, 4, 0.5, 0.0, 10.0, X, lam, B, B, ws, nbytes)          # b0 >= bW
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.cheb_filter(TF32, 0, -2.0, 0.5, 10.0, X, lam, B, B, ws, nbytes)         # m < 1
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.cheb_filter(TF32, 4, -2.0, 0.5, 10.0, X, lam, B - 1, B, ws, nbytes)     # ld < B
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.cheb_filter(TF32, 4, -2.0, 0.5, 10.0, X, lam, B, B, ws, nbytes // 2)    # workspace too small
+    with pytest.raises(PawfeError, match="EINVAL"):
+        ctx.filter_workspace(TF32, 513)                                             # B beyond the maximum
+    torch.cuda.synchronize()
+    assert torch.equal(X, X0)
+    bare = Context(0, torch.cuda.current_stream().cuda_stream)
+    bare.mesh_create(cfg.ncells, cfg.box, cfg.p, PERIODIC, None)
+    Y = torch.empty_like(X)
+    with pytest.raises(PawfeError, match="ESTATE"):
+        bare.apply_H(TF32, X, Y, B, B)                                              # no potential, no atoms yet
+    bare.destroy()
