@@ -68,7 +68,8 @@ pawfe_status launch_dmma_mt(pawfe_ctx* c, const double* A, long cell_stride, con
   auto kern = dmma::k_cell_dmma<RX, CPLX, MT>;
   const size_t smem = dmma::smem_bytes<RX, CPLX, MT>(c->n);
   TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
-  kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+  kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha,
+                                                                                                     nullptr, 0.0, nullptr);
   KERNEL_CHECK(c, "k_cell_dmma");
   return PAWFE_OK;
 }
@@ -221,6 +222,27 @@ pawfe_status pawfe_apply_Sinv_impl(pawfe_ctx* c, const TX* X, long ldx, TY* Y, l
 template <typename RX>
 pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double* Y, long ldy, int B) {
   return launch_dmma<RX, false>(c, (const double*)c->d_H64, (long)c->n * c->n, X, ldx, Y, ldy, B, 1.0);
+}
+// Y += H^e X_e + neg_lam[v] (M^e X_e) in one launch (the mass term as the DMMA accumulators' initial values, cell_dmma.cuh).
+// *done = false (nothing launched) when the shape does not allow it: more than one row block, or the n x 64 staging
+// block does not fit the kernel's ring; the caller then runs the product and k_mass_sf separately.
+// Opt-in (PAWFE_MASSFOLD=1): parity-green, but the gather and the sweeps of 64 columns at one CTA per SM cost 7 ms per
+// config-1 launch (16.5 ms against 9.4 + 2.75 ms for the two kernels), so the separate kernels stay the default.
+pawfe_status pawfe_cell_product_fp64_mass(pawfe_ctx* c, const float* X, long ldx, double* Y, long ldy, int B,
+                                          const double* neg_lam, bool* done) {
+  *done = false;
+  const int n = c->n;
+  if (c->cplx || n <= 224 || n > 352 || !getenv("PAWFE_MASSFOLD")) return PAWFE_OK;
+  constexpr int MT = 11;
+  auto kern = dmma::k_cell_dmma<float, false, MT>;
+  const size_t smem = dmma::smem_bytes<float, false, MT>(n);
+  if ((size_t)n * dmma::kTN * 8 > smem - (size_t)n * 8 - 16) return PAWFE_OK;
+  TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
+  kern<<<(unsigned)ceil_div(B, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(
+      c->md, (const double*)c->d_H64, (long)n * n, X, ldx, Y, ldy, B, 1.0, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, neg_lam);
+  KERNEL_CHECK(c, "k_cell_dmma");
+  *done = true;
+  return PAWFE_OK;
 }
 template pawfe_status pawfe_cell_product_fp64<float>(pawfe_ctx*, const float*, long, double*, long, int);
 template pawfe_status pawfe_cell_product_fp64<double>(pawfe_ctx*, const double*, long, double*, long, int);

@@ -968,14 +968,18 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
     // real: fused (setup_fp64.cuh)
     CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
     FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
-    TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));      // DMMA-bound, on the main stream
+    bool mass_done = false;                                         // DMMA-bound, on the main stream; p <= 6: mass term inside
+    TRY(pawfe_cell_product_fp64_mass(c, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B, &mass_done));
+    if (!mass_done) TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
     {
       StreamSwap sw(c, p->no_aux ? c->stream : p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
-      const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
-      TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float, kMassCT>, smem));
-      k_mass_sf<float, kMassCT><<<dim3(c->ncell, ceil_div(B, kMassCT)), 256, smem, c->stream>>>(
-          c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
-      KERNEL_CHECK(c, "k_mass_sf");
+      if (!mass_done) {
+        const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
+        TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float, kMassCT>, smem));
+        k_mass_sf<float, kMassCT><<<dim3(c->ncell, ceil_div(B, kMassCT)), 256, smem, c->stream>>>(
+            c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
+        KERNEL_CHECK(c, "k_mass_sf");
+      }
       if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
     }
     JOIN_AUX(c, p);

@@ -475,3 +475,23 @@ def test_error_behaviour():
     with pytest.raises(PawfeError, match="ESTATE"):
         bare.apply_H(TF32, X, Y, B, B)                                              # no potential, no atoms yet
     bare.destroy()
+
+
+def test_filter_mass_term_inside_fp64_cell_kernel(monkeypatch):
+    """PAWFE_MASSFOLD=1: the mass part of Y = H X - S X Lambda as the DMMA accumulators' initial values (cell_dmma.cuh)."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import TF32
+    monkeypatch.setenv("PAWFE_MASSFOLD", "1")
+    cfg, sysd, ops, ctx = _setup("cfg1_twin")
+    B, m = 72, 1    # m = 1: the result is the FP64 residual set-up alone, so a mass-term error is not hidden by TF32 noise
+    X0 = random_block(cfg, B, stream=61) * ops.mask[:, None]
+    X = chfsi.s_orthonormalise(ops.apply_S, X0)
+    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
+    b0, bW, bU = _bounds(ops, lam)
+    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+    Xd = _to_dev(X, "tf32", False)
+    nbytes = ctx.filter_workspace(TF32, B)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
+    torch.cuda.synchronize()
+    assert _relerr(_to_host(Xd, False), want) < 5e-5
