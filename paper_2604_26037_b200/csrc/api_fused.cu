@@ -333,6 +333,7 @@ k_scatter2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict_
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int v = blockIdx.y * 128 + lane * 4;
   if (v >= B) return;
+  const bool vec = (ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0;   // rows 16-byte aligned
   float4 wv[PAWFE_MAX_NPJ];
 #pragma unroll
   for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
@@ -349,10 +350,14 @@ k_scatter2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict_
         acc.z = fmaf(cv, wv[al].z, acc.z); acc.w = fmaf(cv, wv[al].w, acc.w);
       }
     float* dst = X + nodeJ[I] * ldx + v;
-    atomicAdd(dst + 0, s * acc.x);
-    if (v + 1 < B) atomicAdd(dst + 1, s * acc.y);
-    if (v + 2 < B) atomicAdd(dst + 2, s * acc.z);
-    if (v + 3 < B) atomicAdd(dst + 3, s * acc.w);
+    if (vec && v + 3 < B) {   // one 16-byte reduction instead of four scalar ones
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(s * acc.x), "f"(s * acc.y), "f"(s * acc.z), "f"(s * acc.w) : "memory");
+    } else {
+      atomicAdd(dst + 0, s * acc.x);
+      if (v + 1 < B) atomicAdd(dst + 1, s * acc.y);
+      if (v + 2 < B) atomicAdd(dst + 2, s * acc.z);
+      if (v + 3 < B) atomicAdd(dst + 3, s * acc.w);
+    }
   }
 }
 
