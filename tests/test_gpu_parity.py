@@ -495,3 +495,23 @@ def test_filter_mass_term_inside_fp64_cell_kernel(monkeypatch):
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
     assert _relerr(_to_host(Xd, False), want) < 5e-5
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32", "tf32"])
+def test_full_loop_eigenvalues_cfg0(prec):
+    """north_star: converged lowest eigenvalues of the full R-ChFSI loop (Algorithm 1 around the library's filter: config 0,
+    degree 10, 30 outer iterations, 16 vectors) within 1e-6 Ha of the oracle's dense FP64 solve eigh(H, S), in every
+    precision mode; Rayleigh-Ritz in FP64 with the library's own applies (paper_2604_26037_b200/harness.py)."""
+    from oracle import chfsi
+    from paper_2604_26037_b200 import PREC
+    from paper_2604_26037_b200.harness import Harness, chfsi_loop
+    cfg, sysd, ops, ctx = _setup("cfg0")
+    want = chfsi.dense_eigh(ops.dense_H(), ops.dense_S())
+    hz = Harness(ctx, ops.mesh.M, cfg.complex)
+    bU = hz.upper_bound(k=10, seed=1)
+    assert bU >= np.max(np.real(np.linalg.eigvals(ops.apply_Sinv(ops.dense_H()))))   # an upper bound of the filtered operator
+    X0 = torch.from_numpy(random_block(cfg, cfg.nvec)).cuda()
+    X, lam = chfsi_loop(ctx, hz, X0, PREC[prec], cfg.degree, bU, cfg.outer)
+    ncheck = (3 * cfg.nvec) // 4     # reading R18
+    err = np.max(np.abs(np.asarray(lam)[:ncheck] - want[:ncheck]))
+    assert err < 1e-6, (prec, err)
