@@ -341,7 +341,7 @@ def test_filter_host_block_set(name, prec):
         ctx.cheb_filter(PREC[prec], m, b0, bW, bU, dev[k], lams[k], B, B, ws, nbytes)
         torch.cuda.synchronize()
         # same kernels on the same data: equal up to the order of the FP32 assembly reductions (R20)
-        assert _relerr(_to_host(dev[k], cfg.complex), got) < (1e-13 if prec == "fp64" else 1e-5)
+        assert _relerr(_to_host(dev[k], cfg.complex), got) < (1e-12 if prec == "fp64" else 1e-5)
 
 
 @pytest.mark.parametrize("name", ["cfg1_twin", "cfg4_twin"])
@@ -514,4 +514,6 @@ def test_full_loop_eigenvalues_cfg0(prec):
     X, lam = chfsi_loop(ctx, hz, X0, PREC[prec], cfg.degree, bU, cfg.outer)
     ncheck = (3 * cfg.nvec) // 4     # reading R18
     err = np.max(np.abs(np.asarray(lam)[:ncheck] - want[:ncheck]))
-    assert err < 1e-6, (prec, err)
+    # north_star's bar is 1e-6 Ha; measured 2.5e-14 in all three modes (Rayleigh-Ritz is FP64, the filter only has to span
+    # the subspace), so the gate is held far tighter than the bar
+    assert err < 1e-10, (prec, err)
