@@ -22,5 +22,10 @@ Pins (tests/test_oracle_*.py, ``-m "not gpu"``) -- see DESIGN.md "Oracle pins":
   filter (Alg. 2) ............ == plain Chebyshev filter Eq. 19-20 with exact S^-1; eigenpair fixed point
   outer loop (Alg. 1) ........ lowest Ritz values == dense eigh(H, S) on config 0
   complex path ............... H(k) Hermitian, k=0 reproduces real matrices, 1/2|k+G|^2 spectrum
-No function on the path is "parity unpinned".
+Round 2 (tests/test_oracle_pins_r2.py; each verified to turn red under the mutation named):
+  potential cell matrix ...... 0th / 1st / 2nd moments of V^e == closed Gaussian moments (x<->z mirror of the points)
+  lumped mass ................ composite GLL rule: exact to degree 2p-1, Lobatto remainder at 2p (uniform weights)
+  k-term of H^e .............. k with three different components, per-axis +-G plane waves (G_x <-> G_z swap)
+  operators.apply_H_rows ..... == rows of the assembled product on config 0, complex and Dirichlet twins (dropped cell)
+With these, no function on the path is "parity unpinned".
 """
