@@ -18,8 +18,10 @@
  *  - Every function returns a pawfe_status and never throws across the ABI; pawfe_last_error()
  *    gives the text of the last failure on that context.
  *  - "host" / "device" is stated for every pointer.  Device pointers must belong to the context's
- *    device.  All work is enqueued on the context's CUDA stream; hot calls (apply_*, cheb_filter,
- *    col_norms, axpy helpers) allocate nothing and do not synchronise the host, except where stated.
+ *    device.  All work is enqueued on the context's CUDA stream.  Hot calls (apply_*, cheb_filter*, col_norms) do not
+ *    synchronise the host and allocate nothing ONCE pawfe_prepare has been called for their (prec, B, m); without it
+ *    the library's internal plans and scratch (re-tiled operand streams, projection scratch, coefficient staging) are
+ *    built on the first call that needs them and re-grown when a wider block arrives, which synchronises the stream.
  *  - The library OWNS the operators (cell matrices, projector blocks, couplings, lumped mass) and
  *    frees them in pawfe_destroy.  The CALLER owns all vector blocks and the filter workspace.
  *  - Vector blocks are row-major [dof][vec] ("vec" contiguous), leading dimension ld in ELEMENTS.
@@ -94,6 +96,13 @@ pawfe_status pawfe_mesh_create(pawfe_ctx* ctx, const int ncells[3], const double
 pawfe_status pawfe_local_potential_gaussians(pawfe_ctx* ctx, int natoms, const double* pos,
                                              const double* Z, const double* sigma, int keep_fp64);
 
+/* Cell matrices supplied by the caller instead (e.g. built by an independent implementation, to run the library's
+ * kernels on them): Hcell = [cell][I][J] doubles, cell = (cx*ncy + cy)*ncz + cz, I = (a*(p+1) + b)*(p+1) + c, complex
+ * contexts interleaved (re, im); host (is_device = 0) or device memory.  Replaces H^e of every cell; the mass cell
+ * matrix stays the mesh's M^e = (hx hy hz / 8) M1 x M1 x M1.  FP32 copies are derived; keep_fp64 as above.
+ * Synchronises the host. */
+pawfe_status pawfe_set_cell_matrices(pawfe_ctx* ctx, const double* Hcell, int is_device, int keep_fp64);
+
 /* ---- atoms and projectors (Eq. 16-17; Eq. 34; Eq. 28-29) ----------- */
 
 /* One species: nproj projectors p_alpha(d) = amp * r^l exp(-r^2 / 2 sigma^2) (1-(r/rc)^2)^2 Y_lm(d/r)
@@ -108,6 +117,14 @@ pawfe_status pawfe_local_potential_gaussians(pawfe_ctx* ctx, int natoms, const d
 pawfe_status pawfe_atoms_create(pawfe_ctx* ctx, int natoms, const double* pos, int nproj,
                                 const int* proj_l, const int* proj_m, const double* proj_sigma,
                                 const double* proj_amp, double rc, const double* D, const double* dS);
+
+/* The (cell, atom) pairs the library holds projector blocks for, in its own order (pairs sorted by atom, then cell):
+ * pair_cell, pair_atom: host, pawfe_num_pairs ints each. */
+pawfe_status pawfe_get_pairs(pawfe_ctx* ctx, int* pair_cell, int* pair_atom);
+/* Projector blocks supplied by the caller for exactly those pairs: Cd = [pair][alpha][I] doubles = (C^{e,a dagger})_{alpha I}
+ * (Eq. 34; complex interleaved), host or device.  G^a, Delta^a_Sinv and the FP32 copies are rebuilt from them.
+ * Synchronises the host. */
+pawfe_status pawfe_set_projector_blocks(pawfe_ctx* ctx, const double* Cd, int is_device);
 
 /* Replace D (Delta_H changes every SCF step, Eq. 18).  host, natoms*nproj*nproj. */
 pawfe_status pawfe_update_coupling(pawfe_ctx* ctx, const double* D);
@@ -130,10 +147,19 @@ pawfe_status pawfe_get_sinv_coupling(pawfe_ctx* ctx, double* out_host);
 pawfe_status pawfe_apply_H(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
 pawfe_status pawfe_apply_S(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
 pawfe_status pawfe_apply_Sinv(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+/* Y = H S^-1approx X, the operator Algorithm 2 iterates (Alg. 1 step 2 L244; Eq. 30; T of Eq. 39 L367 is never
+ * stored).  FP32 / TF32 blocks with 16-byte aligned X, Y and ld, B multiples of 4 (complex: of 2) run exactly the kernel
+ * sequence of one filter step (projection, couplings, one cell contraction with the low-rank terms inside). */
+pawfe_status pawfe_apply_HSinv(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+
+/* Build every internal plan and scratch array the hot calls need for blocks of up to Bmax vectors, Chebyshev degree up to
+ * mmax, in precision mode prec (see Conventions).  Optional; synchronises the host.  Call again after the operators
+ * change or for a wider block. */
+pawfe_status pawfe_prepare(pawfe_ctx* ctx, pawfe_prec prec, int Bmax, int mmax);
 
 /* ---- Algorithm 2 (L250-L282) --------------------------------------------------------------- */
 
-/* Bytes of device workspace pawfe_cheb_filter needs for block width B (leading dimension B). */
+/* Bytes of device workspace pawfe_cheb_filter needs for block width B (any leading dimension, any alignment of X). */
 pawfe_status pawfe_filter_workspace(pawfe_ctx* ctx, pawfe_prec prec, int B, size_t* bytes);
 
 /* Residual-based Chebyshev filter of degree m >= 1:
@@ -147,10 +173,19 @@ pawfe_status pawfe_filter_workspace(pawfe_ctx* ctx, pawfe_prec prec, int B, size
  *   step 5  X <- S^-1approx R_Y + X Lambda_Y                                                    (L282)
  * X: device, in Psi_in / out Psi_f, [dof][vec], leading dimension ld, element type by prec.
  * lambda: HOST, B doubles.  workspace: device, >= pawfe_filter_workspace bytes, 256-byte aligned.
- * The B scalars are copied to the device asynchronously from an internal pinned buffer. */
+ * Needs b0 < bW < bU (strictly: a one-vector block needs bW above its Ritz value) and 1 <= m <= 512; PAWFE_EINVAL otherwise.
+ * The B scalars are copied to the device asynchronously from an internal pinned buffer (the call waits on the host only
+ * for the staging slot used four calls earlier). */
 pawfe_status pawfe_cheb_filter(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW, double bU,
                                void* X, const double* lambda, long ld, int B,
                                void* workspace, size_t workspace_bytes);
+
+/* Algorithm 2 with step 2 taken from products the caller already holds: HX = H Psi_in and SX = S Psi_in (device, FP64
+ * scalars, layout and leading dimension of X; complex interleaved), e.g. the H Psi_f Q, S Psi_f Q of the last Rayleigh-Ritz
+ * step (L402-L408): Y = HX - SX Lambda costs no operator application (L260, L290).  Everything else as pawfe_cheb_filter. */
+pawfe_status pawfe_cheb_filter_hs(pawfe_ctx* ctx, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                  void* X, const double* HX, const double* SX, const double* lambda, long ld, int B,
+                                  void* workspace, size_t workspace_bytes);
 
 /* Same call with HOST vector block X_host (B columns, leading dimension ld): copies it to an
  * internal device block, filters, copies Psi_f back, and synchronises.  The internal block and

@@ -27,7 +27,8 @@ SYMBOLS = [
     "pawfe_num_pairs", "pawfe_get_cell_matrix", "pawfe_get_sinv_coupling", "pawfe_apply_H", "pawfe_apply_S",
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
-    "pawfe_cell_timing_read",
+    "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
+    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs",
 ]
 
 
@@ -62,7 +63,13 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_num_pairs.argtypes = [vp, C.POINTER(C.c_long)]
     lib.pawfe_get_cell_matrix.argtypes = [vp, C.c_long, dp]
     lib.pawfe_get_sinv_coupling.argtypes = [vp, dp]
-    for f in (lib.pawfe_apply_H, lib.pawfe_apply_S, lib.pawfe_apply_Sinv):
+    lib.pawfe_set_cell_matrices.argtypes = [vp, vp, C.c_int, C.c_int]
+    lib.pawfe_get_pairs.argtypes = [vp, ip, ip]
+    lib.pawfe_set_projector_blocks.argtypes = [vp, vp, C.c_int]
+    lib.pawfe_prepare.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+    lib.pawfe_cheb_filter_hs.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp, dp,
+                                         C.c_long, C.c_int, vp, C.c_size_t]
+    for f in (lib.pawfe_apply_H, lib.pawfe_apply_S, lib.pawfe_apply_Sinv, lib.pawfe_apply_HSinv):
         f.argtypes = [vp, C.c_int, vp, vp, C.c_long, C.c_int]
     lib.pawfe_filter_workspace.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_size_t)]
     lib.pawfe_cheb_filter.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, dp,
@@ -156,6 +163,27 @@ class Context:
                                                 _iptr(m), _dptr(sg), _dptr(am), float(rc), _dptr(D), _dptr(dS)),
                     "pawfe_atoms_create")
 
+    def set_cell_matrices(self, Hcell: np.ndarray, keep_fp64: bool = True):
+        """Hcell: host array [cell][n][n], float64 or complex128 (pawfe_set_cell_matrices)."""
+        H = np.ascontiguousarray(Hcell, dtype=np.complex128 if self.complex else np.float64)
+        self._check(self.lib.pawfe_set_cell_matrices(self._h, C.c_void_p(H.ctypes.data), 0, int(keep_fp64)),
+                    "pawfe_set_cell_matrices")
+
+    def get_pairs(self):
+        n = self.num_pairs()
+        pc, pa = np.zeros(max(n, 1), dtype=np.int32), np.zeros(max(n, 1), dtype=np.int32)
+        self._check(self.lib.pawfe_get_pairs(self._h, _iptr(pc), _iptr(pa)), "pawfe_get_pairs")
+        return pc[:n], pa[:n]
+
+    def set_projector_blocks(self, Cd: np.ndarray):
+        """Cd: host array [pair][nproj][n], float64 or complex128 (pawfe_set_projector_blocks)."""
+        A = np.ascontiguousarray(Cd, dtype=np.complex128 if self.complex else np.float64)
+        self._check(self.lib.pawfe_set_projector_blocks(self._h, C.c_void_p(A.ctypes.data), 0),
+                    "pawfe_set_projector_blocks")
+
+    def prepare(self, prec: int, Bmax: int, mmax: int):
+        self._check(self.lib.pawfe_prepare(self._h, int(prec), int(Bmax), int(mmax)), "pawfe_prepare")
+
     def update_coupling(self, D):
         D = _f64(D)
         self._check(self.lib.pawfe_update_coupling(self._h, _dptr(D)), "pawfe_update_coupling")
@@ -210,6 +238,16 @@ class Context:
 
     def apply_Sinv(self, prec: int, X, Y, ld: int, B: int):
         self._check(self.lib.pawfe_apply_Sinv(self._h, int(prec), self._ptr(X), self._ptr(Y), int(ld), int(B)), "pawfe_apply_Sinv")
+
+    def apply_HSinv(self, prec: int, X, Y, ld: int, B: int):
+        self._check(self.lib.pawfe_apply_HSinv(self._h, int(prec), self._ptr(X), self._ptr(Y), int(ld), int(B)), "pawfe_apply_HSinv")
+
+    def cheb_filter_hs(self, prec: int, m: int, b0: float, bW: float, bU: float, X, HX, SX, lam, ld: int, B: int,
+                       workspace, workspace_bytes: int):
+        lam = _f64(lam)
+        self._check(self.lib.pawfe_cheb_filter_hs(self._h, int(prec), int(m), float(b0), float(bW), float(bU),
+                                                  self._ptr(X), self._ptr(HX), self._ptr(SX), _dptr(lam), int(ld), int(B),
+                                                  self._ptr(workspace), int(workspace_bytes)), "pawfe_cheb_filter_hs")
 
     def filter_workspace(self, prec: int, B: int) -> int:
         v = C.c_size_t()

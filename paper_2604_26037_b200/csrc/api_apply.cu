@@ -68,8 +68,7 @@ pawfe_status launch_dmma_mt(pawfe_ctx* c, const double* A, long cell_stride, con
   auto kern = dmma::k_cell_dmma<RX, CPLX, MT>;
   const size_t smem = dmma::smem_bytes<RX, CPLX, MT>(c->n);
   TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
-  kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha,
-                                                                                                     nullptr, 0.0, nullptr);
+  kern<<<(unsigned)ceil_div(Wr, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(c->md, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   KERNEL_CHECK(c, "k_cell_dmma");
   return PAWFE_OK;
 }
@@ -82,11 +81,8 @@ pawfe_status launch_dmma(pawfe_ctx* c, const double* A, long cell_stride, const 
   if (n <= 128) return launch_dmma_mt<RX, CPLX, 4>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   if (n <= 224) return launch_dmma_mt<RX, CPLX, 7>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   if (n <= 352) {
-    // n = 343 (p = 6): MT = 6 is two row blocks (192 + 151 rows) at two CTAs per SM, MT = 11 one row block at one CTA per SM
-    const char* d = getenv("PAWFE_DMMA_MT");   // timing experiments
-    const int mt = d ? atoi(d) : 0;
-    if (mt == 5) return launch_dmma_mt<RX, CPLX, 5>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
-    if (mt == 6) return launch_dmma_mt<RX, CPLX, 6>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
+    // n = 343 (p = 6): MT = 11 is one row block at one CTA per SM (two row blocks at two CTAs per SM, MT = 5 / 6, were not
+    // faster: DESIGN.md section 7)
     return launch_dmma_mt<RX, CPLX, 11>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
   }
   return launch_dmma_mt<RX, CPLX, 8>(c, A, cell_stride, X, ldx, Y, ldy, Wr, alpha);
@@ -223,27 +219,6 @@ template <typename RX>
 pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double* Y, long ldy, int B) {
   return launch_dmma<RX, false>(c, (const double*)c->d_H64, (long)c->n * c->n, X, ldx, Y, ldy, B, 1.0);
 }
-// Y += H^e X_e + neg_lam[v] (M^e X_e) in one launch (the mass term as the DMMA accumulators' initial values, cell_dmma.cuh).
-// *done = false (nothing launched) when the shape does not allow it: more than one row block, or the n x 64 staging
-// block does not fit the kernel's ring; the caller then runs the product and k_mass_sf separately.
-// Opt-in (PAWFE_MASSFOLD=1): parity-green, but the gather and the sweeps of 64 columns at one CTA per SM cost 7 ms per
-// config-1 launch (16.5 ms against 9.4 + 2.75 ms for the two kernels), so the separate kernels stay the default.
-pawfe_status pawfe_cell_product_fp64_mass(pawfe_ctx* c, const float* X, long ldx, double* Y, long ldy, int B,
-                                          const double* neg_lam, bool* done) {
-  *done = false;
-  const int n = c->n;
-  if (c->cplx || n <= 224 || n > 352 || !getenv("PAWFE_MASSFOLD")) return PAWFE_OK;
-  constexpr int MT = 11;
-  auto kern = dmma::k_cell_dmma<float, false, MT>;
-  const size_t smem = dmma::smem_bytes<float, false, MT>(n);
-  if ((size_t)n * dmma::kTN * 8 > smem - (size_t)n * 8 - 16) return PAWFE_OK;
-  TRY(pawfe_ensure_smem(c, (const void*)kern, smem));
-  kern<<<(unsigned)ceil_div(B, dmma::kTN) * (unsigned)c->ncell, dmma::kThreads, smem, c->stream>>>(
-      c->md, (const double*)c->d_H64, (long)n * n, X, ldx, Y, ldy, B, 1.0, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, neg_lam);
-  KERNEL_CHECK(c, "k_cell_dmma");
-  *done = true;
-  return PAWFE_OK;
-}
 template pawfe_status pawfe_cell_product_fp64<float>(pawfe_ctx*, const float*, long, double*, long, int);
 template pawfe_status pawfe_cell_product_fp64<double>(pawfe_ctx*, const double*, long, double*, long, int);
 
@@ -325,10 +300,11 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
     if (tc_usable(c, X, 2 * ldx, Y, 2 * ldy, 2 * B) && fused_supported(c, prec, B))
       return fused_apply_H(c, prec, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, B);
     if (tf32 && tc_usable(c, X, 2 * ldx, Y, 2 * ldy, 2 * B)) {
-      // complex TF32: interleaved (re, im) columns as a real block of 2B columns; P / Q accumulators in the kernel
-      TRY(zero_block(c, (float2*)Y, ldy, B));
+      // complex TF32: interleaved (re, im) columns as a real block of 2B columns; P / Q accumulators in the kernel;
+      // every row is stored by its first writer (no zero fill)
+      TcEpi st_epi; st_epi.mode = TC_EPI_STORE; st_epi.Yt = nullptr; st_epi.aLam = nullptr; st_epi.ac = st_epi.zz1 = 0.f; st_epi.cw = 2;
       prof_begin(c);
-      pawfe_status st = tc_cell_apply(c, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, 2 * B, 1.0f);
+      pawfe_status st = tc_cell_apply(c, (const float*)X, 2 * ldx, (float*)Y, 2 * ldy, 2 * B, 1.0f, nullptr, &st_epi);
       prof_end(c);
       TRY(st);
       return pawfe_apply_nonlocal<float2, float2, float2>(c, OpData<float2>::D(c), 1.0, (const float2*)X, ldx, 0, (float2*)Y, ldy, 0, B, nullptr);
@@ -338,14 +314,39 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
   if (tc_usable(c, X, ldx, Y, ldy, B) && fused_supported(c, prec, B))
     return fused_apply_H(c, prec, (const float*)X, ldx, (float*)Y, ldy, B);
   if (tf32 && tc_usable(c, X, ldx, Y, ldy, B)) {
-    TRY(zero_block(c, (float*)Y, ldy, B));
+    TcEpi st_epi; st_epi.mode = TC_EPI_STORE; st_epi.Yt = nullptr; st_epi.aLam = nullptr; st_epi.ac = st_epi.zz1 = 0.f; st_epi.cw = 1;
     prof_begin(c);
-    pawfe_status st = tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f);
+    pawfe_status st = tc_cell_apply(c, (const float*)X, ldx, (float*)Y, ldy, B, 1.0f, nullptr, &st_epi);
     prof_end(c);
     TRY(st);
     return pawfe_apply_nonlocal<float, float, float>(c, OpData<float>::D(c), 1.0, (const float*)X, ldx, 0, (float*)Y, ldy, 0, B, nullptr);
   }
   return pawfe_apply_HS<float, float, float>(c, 0, tf32, (const float*)X, ldx, (float*)Y, ldy, B);
+}
+
+// Y = H S^-1approx X.  FP32 / TF32 blocks that meet the tensor-core kernel's alignment rules run the fused step's kernel
+// configuration (fused_apply_HSinv); everything else S^-1approx then H through a context-owned block T.
+extern "C" pawfe_status pawfe_apply_HSinv(pawfe_ctx* c, pawfe_prec prec, const void* X, void* Y, long ld, int B) {
+  TRY(check_apply(c, prec, X, Y, ld, B, true));
+  const int cw = c->cplx ? 2 : 1;
+  if (prec != PAWFE_FP64 && tc_usable(c, X, cw * ld, Y, cw * ld, cw * B) && fused_supported(c, prec, B))
+    return fused_apply_HSinv(c, prec, (const float*)X, cw * ld, (float*)Y, cw * ld, B);
+  const size_t es = (prec == PAWFE_FP64 ? 8 : 4) * (size_t)cw;
+  const size_t need = (size_t)c->M * B * es;
+  if (need > c->tmpblk_bytes) {   // first use / wider block (pawfe_prepare sizes it ahead)
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_tmpblk); c->d_tmpblk = nullptr; c->tmpblk_bytes = 0;
+    char* q = nullptr; TRY(dev_alloc(c, &q, need)); c->d_tmpblk = q; c->tmpblk_bytes = need;
+  }
+  void* T = c->d_tmpblk;
+  if (c->cplx) {
+    if (prec == PAWFE_FP64) TRY((pawfe_apply_Sinv_impl<double2, double2, double2>(c, (const double2*)X, ld, (double2*)T, B, B)));
+    else TRY((pawfe_apply_Sinv_impl<float2, float2, float2>(c, (const float2*)X, ld, (float2*)T, B, B)));
+  } else {
+    if (prec == PAWFE_FP64) TRY((pawfe_apply_Sinv_impl<double, double, double>(c, (const double*)X, ld, (double*)T, B, B)));
+    else TRY((pawfe_apply_Sinv_impl<float, float, float>(c, (const float*)X, ld, (float*)T, B, B)));
+  }
+  return pawfe_apply_H_any(c, prec, T, B, Y, ld, B);
 }
 
 extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec prec, int B) {

@@ -6,6 +6,7 @@
 #include "fe_setup.cuh"
 #include "kernels_simt.cuh"
 #include "api_internal.h"
+#include "fused.h"
 #include <algorithm>
 #include <cmath>
 
@@ -225,6 +226,40 @@ extern "C" pawfe_status pawfe_atoms_create(pawfe_ctx* c, int natoms, const doubl
   TRY(pawfe_upload_couplings(c, D, dS, G));
   c->have_atoms = true;
   return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_get_pairs(pawfe_ctx* c, int* pair_cell, int* pair_atom) {
+  if (!c || !pair_cell || !pair_atom) return PAWFE_EINVAL;
+  if (!c->have_atoms) return PAWFE_ESTATE;
+  if (c->npairs == 0) return PAWFE_OK;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  CUDA_TRY(c, cudaMemcpy(pair_cell, c->d_pair_cell, c->npairs * sizeof(int), cudaMemcpyDeviceToHost));
+  CUDA_TRY(c, cudaMemcpy(pair_atom, c->d_pair_atom, c->npairs * sizeof(int), cudaMemcpyDeviceToHost));
+  return PAWFE_OK;
+}
+
+// User- (or oracle-) built projector blocks for the library's pair list: replaces C^{e,a dagger}, then G^a, Delta_Sinv
+// and the FP32 copies are rebuilt from them exactly as pawfe_atoms_create does.
+extern "C" pawfe_status pawfe_set_projector_blocks(pawfe_ctx* c, const double* Cd, int is_device) {
+  if (!c || !Cd) return PAWFE_EINVAL;
+  if (!c->have_atoms) return PAWFE_ESTATE;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  fused_invalidate(c);
+  const int cw = c->cplx ? 2 : 1;
+  const size_t celems = (size_t)c->npairs * c->npj * c->n * cw;
+  if (celems > 0) {
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_Cd64, Cd, celems * sizeof(double), is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    k_f64_to_f32<<<4 * c->sm_count, 256, 0, c->stream>>>((const double*)c->d_Cd64, (float*)c->d_Cd32, (long)celems);
+    KERNEL_CHECK(c, "k_f64_to_f32");
+  }
+  std::vector<double> G((size_t)c->natoms * c->npj * c->npj * cw, 0.0);
+  if (c->npairs > 0) {
+    if (c->cplx) TRY(compute_G<double2>(c, G)); else TRY(compute_G<double>(c, G));
+  }
+  c->h_G = G;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return pawfe_upload_couplings(c, nullptr, c->h_dS.data(), G);
 }
 
 extern "C" pawfe_status pawfe_update_coupling(pawfe_ctx* c, const double* D) {

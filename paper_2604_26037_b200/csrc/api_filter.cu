@@ -7,6 +7,7 @@
 #include "api_internal.h"
 #include "apply_impl.h"
 #include "fused.h"
+#include "setup_fp64.cuh"
 #include <algorithm>
 #include <cstring>
 #include <type_traits>
@@ -97,7 +98,8 @@ pawfe_status filter_scalars(pawfe_ctx* c, int m, double b0, double bW, double bU
 // TS: storage scalar (float / double / float2 / double2), TD: FP64 scalar of the same kind
 template <typename TS, typename TD>
 pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU, TS* X,
-                         const double* lambda, long ld, int B, void* workspace) {
+                         const double* lambda, long ld, int B, void* workspace, const void* HXin = nullptr,
+                         const void* SXin = nullptr) {
   typedef typename ScalarTraits<TS>::real RS;
   const int cw = ScalarTraits<TS>::cplx ? 2 : 1;
   const int W = B * cw;
@@ -117,11 +119,16 @@ pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double
   const std::vector<double>&as = fs.as, &acs = fs.acs, &zzs = fs.zzs;
   const double z_over_e = fs.z_over_e;
 
-  // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
-  TRY((pawfe_apply_HS<TS, TD, TD>(c, 0, false, X, ld, Y64, B, B)));
-  (void)SX64;   // S X is not stored: Y -= (S X) Lambda directly (mass part by 1-D sweeps, Lambda folded into the coupling)
-  TRY((pawfe_sub_SX_lambda<TS, TD>(c, X, ld, Y64, B, B, ds, ds + (size_t)(m + 1) * B)));
   const int gs = 8 * c->sm_count;
+  // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
+  if (HXin && SXin) {   // the caller's products (pawfe_cheb_filter_hs): no operator application
+    k_residual_from_products<<<gs, 256, 0, c->stream>>>(c->M, (long)W, W, cw, (const double*)HXin, (const double*)SXin, ld * cw, ds, (double*)Y64);
+    KERNEL_CHECK(c, "k_residual_from_products");
+  } else {
+    TRY((pawfe_apply_HS<TS, TD, TD>(c, 0, false, X, ld, Y64, B, B)));
+    (void)SX64;   // S X is not stored: Y -= (S X) Lambda directly (mass part by 1-D sweeps, Lambda folded into the coupling)
+    TRY((pawfe_sub_SX_lambda<TS, TD>(c, X, ld, Y64, B, B, ds, ds + (size_t)(m + 1) * B)));
+  }
   // ---- step 3 ----
   k_residual_init<RS><<<gs, 256, 0, c->stream>>>(c->M, W, cw, (double*)Y64, (const double*)nullptr, ds, z_over_e,
                                                  (RS*)RX, (RS*)RY);
@@ -184,14 +191,38 @@ bool fused_width_ok(pawfe_ctx* c, pawfe_prec prec, int B) { return fused_support
 extern "C" pawfe_status pawfe_filter_workspace(pawfe_ctx* c, pawfe_prec prec, int B, size_t* bytes) {
   if (!c || !bytes || B < 1 || B > 512) return PAWFE_EINVAL;
   if (!c->have_mesh) return PAWFE_ESTATE;
-  *bytes = filter_ws_bytes(c, prec, B, fused_width_ok(c, prec, B));
+  // complex blocks with an odd leading dimension or a misaligned pointer fall back to the unfused sequence, which needs
+  // more: complex contexts are always told the larger figure, so a workspace of this size fits every (ld, X)
+  const size_t fused = filter_ws_bytes(c, prec, B, fused_width_ok(c, prec, B));
+  *bytes = c->cplx ? std::max(fused, filter_ws_bytes(c, prec, B, false)) : fused;
   return PAWFE_OK;
 }
 
-extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
-                                          void* X, const double* lambda, long ld, int B, void* workspace,
-                                          size_t workspace_bytes) {
+// Allocate now what the hot calls would otherwise allocate on first use (include/pawfe.h).
+extern "C" pawfe_status pawfe_prepare(pawfe_ctx* c, pawfe_prec prec, int Bmax, int mmax) {
+  if (!c || Bmax < 1 || Bmax > 512 || mmax < 1 || mmax > 512) return PAWFE_EINVAL;
+  if (prec != PAWFE_FP64 && prec != PAWFE_FP32 && prec != PAWFE_TF32) return PAWFE_EINVAL;
+  if (!c->have_mesh || !c->have_atoms || !c->have_pot) { c->err = "operators not set up"; return PAWFE_ESTATE; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  TRY(ensure_scalars(c, (size_t)(mmax + 2) * Bmax));
+  TRY(pawfe_ensure_P(c, Bmax));
+  if (prec != PAWFE_FP64 && tc_supported(c, Bmax)) TRY(tc_prepare(c));
+  if (fused_supported(c, prec, Bmax)) TRY(fused_prepare_all(c, prec, Bmax, true));
+  const size_t need = (size_t)c->M * Bmax * (prec == PAWFE_FP64 ? 8 : 4) * (c->cplx ? 2 : 1);
+  if (need > c->tmpblk_bytes) {
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_tmpblk); c->d_tmpblk = nullptr; c->tmpblk_bytes = 0;
+    char* q = nullptr; TRY(dev_alloc(c, &q, need)); c->d_tmpblk = q; c->tmpblk_bytes = need;
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return PAWFE_OK;
+}
+
+static pawfe_status cheb_filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                     void* X, const double* lambda, long ld, int B, void* workspace,
+                                     size_t workspace_bytes, const void* HX, const void* SX) {
   TRY(check_filter(c, prec, m, b0, bW, bU, X, lambda, ld, B));
+  if ((HX != nullptr) != (SX != nullptr)) { c->err = "give both H X and S X, or neither"; return PAWFE_EINVAL; }
   // complex blocks with an odd leading dimension or a misaligned pointer run the generic sequence (larger workspace)
   const bool fused = fused_width_ok(c, prec, B) && (!c->cplx || (!(ld & 1) && !((uintptr_t)X & 15)));
   const size_t need = filter_ws_bytes(c, prec, B, fused);
@@ -202,21 +233,36 @@ extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, 
   }
   CUDA_TRY(c, cudaSetDevice(c->device));
   if (c->cplx) {
-    if (prec == PAWFE_FP64) return filter_impl<double2, double2>(c, prec, m, b0, bW, bU, (double2*)X, lambda, ld, B, workspace);
+    if (prec == PAWFE_FP64) return filter_impl<double2, double2>(c, prec, m, b0, bW, bU, (double2*)X, lambda, ld, B, workspace, HX, SX);
     if (fused) {
       FilterScalars fs;
       TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
-      return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace);
+      return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace, HX, SX);
     }
-    return filter_impl<float2, double2>(c, prec, m, b0, bW, bU, (float2*)X, lambda, ld, B, workspace);
+    return filter_impl<float2, double2>(c, prec, m, b0, bW, bU, (float2*)X, lambda, ld, B, workspace, HX, SX);
   }
-  if (prec == PAWFE_FP64) return filter_impl<double, double>(c, prec, m, b0, bW, bU, (double*)X, lambda, ld, B, workspace);
+  if (prec == PAWFE_FP64) return filter_impl<double, double>(c, prec, m, b0, bW, bU, (double*)X, lambda, ld, B, workspace, HX, SX);
   if (fused) {
     FilterScalars fs;
     TRY(filter_scalars(c, m, b0, bW, bU, lambda, B, &fs));
-    return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace);
+    return fused_filter(c, prec, m, fs.ds, fs.as.data(), fs.acs.data(), fs.zzs.data(), fs.z_over_e, X, ld, B, workspace, HX, SX);
   }
-  return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace);
+  return filter_impl<float, double>(c, prec, m, b0, bW, bU, (float*)X, lambda, ld, B, workspace, HX, SX);
+}
+
+extern "C" pawfe_status pawfe_cheb_filter(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                          void* X, const double* lambda, long ld, int B, void* workspace,
+                                          size_t workspace_bytes) {
+  return cheb_filter_impl(c, prec, m, b0, bW, bU, X, lambda, ld, B, workspace, workspace_bytes, nullptr, nullptr);
+}
+
+// Algorithm 2 with step 2 taken from products the caller already holds
+extern "C" pawfe_status pawfe_cheb_filter_hs(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW, double bU,
+                                             void* X, const double* HX, const double* SX, const double* lambda, long ld,
+                                             int B, void* workspace, size_t workspace_bytes) {
+  if (!c) return PAWFE_EINVAL;
+  if (!HX || !SX) { c->err = "pawfe_cheb_filter_hs needs H X and S X"; return PAWFE_EINVAL; }
+  return cheb_filter_impl(c, prec, m, b0, bW, bU, X, lambda, ld, B, workspace, workspace_bytes, HX, SX);
 }
 
 extern "C" pawfe_status pawfe_cheb_filter_host(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double bW,

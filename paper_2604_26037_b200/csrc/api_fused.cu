@@ -1,6 +1,7 @@
-// api_fused.cu -- fused Chebyshev step of Algorithm 2 for real FP32-storage blocks (see fused.h, DESIGN.md
-// "Fused step"): plan construction (K-extension blocks, neighbour couplings), the atom-local projection and
-// coupling kernels (Fig. 2 step ii; Eq. 28-29), the bracket prepass (L272, L374), recovery (L282).
+// api_fused.cu -- fused Chebyshev step of Algorithm 2 for FP32-storage blocks (see fused.h):
+// plan construction (K-extension blocks, neighbour couplings), the atom-local projection and coupling kernels
+// (Fig. 2 step ii; Eq. 28-29), the step loop (the bracket of L272 / L374 is written by the cell kernel's
+// first writers, cell_tcgen05.cu), recovery (L282).
 #include "fused.h"
 #include "cell_tcgen05.h"
 #include "host_util.h"
@@ -8,6 +9,7 @@
 #include "apply_impl.h"
 #include "setup_fp64.cuh"
 #include "nonlocal_f32.cuh"
+#include "kernels_stream.cuh"
 #include <algorithm>
 #include <cmath>
 #include <set>
@@ -23,7 +25,6 @@ struct FusedPlan {
   float* d_GD = nullptr;        // [nnb][npj][npj]:  G^{ab} Delta^b_Sinv
   int* d_cps = nullptr;         // [ncell + 1] cell -> its (cell, atom) pairs
   int* d_cpi = nullptr;         // [npairs] pair indices by cell
-  bool ppfuse = false;          // PAWFE_PPFUSE=1: bracket and projection in one sweep (k_prepass_proj; slower so far)
   int ext_ksteps = 4;
   // scratch for block width <= Bcap
   int Bcap = 0; long ldw = 0;
@@ -31,7 +32,8 @@ struct FusedPlan {
   float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
   float* d_Wcat_lo = nullptr;   // low parts of Wcat (FP32 mode, 3xTF32 split)
   float* d_Bext_lo = nullptr;   // low parts of d_Bext (built on first FP32-mode use)
-  float* d_xlo = nullptr; size_t xlo_elems = 0;   // low parts of the input block of fused_apply_H in FP32 mode
+  float* d_xlo = nullptr; size_t xlo_elems = 0;   // low parts of the input block of fused_apply_H / _HSinv in FP32 mode
+  float* d_xs = nullptr; size_t xs_elems = 0;     // M_D^-1 X of fused_apply_HSinv
   // second stream for work that is independent inside a step (projection || bracket prepass; mass / non-local || DMMA)
   cudaStream_t aux = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   bool no_aux = false;          // PAWFE_NO_AUX=1: everything on the context's stream (timing experiments)
@@ -259,21 +261,22 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
 // Couplings per atom and vector (Eq. 28-29, Eq. 16):
 //   W^a = Delta^a_Sinv P1^a;  P2^a = P1^a - sum_{b in nb(a)} (G^{ab} Delta^b_Sinv) P1^b;  W2^a = D^a P2^a.
 //   mode 0: both (filter step);  mode 1: W only (recovery, S^-1approx alone);  mode 2: plain H (W = 0, W2 = D P1).
-//   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2.  grid = (natoms, ceil(B/32)), block = 32 * npj: one thread per
+//   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2; columns B <= v < Bpad (the pad columns of a ragged block the cell
+//   kernel's 16-byte gathers touch) are written as 0.  grid = (natoms, ceil(Bpad/32)), block = 32 * npj: one thread per
 //   (output row al, vector), so the dependent chain per thread is one dot product per neighbour instead of npj of them;
 //   P2 goes through shared memory for the last product.
 // ------------------------------------------------------------------------------------------------
 constexpr int kCoupleLanes = 32;
 template <typename T>   // float (real context) or float2 (complex context); ldp, ldw in units of T
 __global__ void __launch_bounds__(kCoupleLanes * PAWFE_MAX_NPJ)
-k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, const T* __restrict__ dSinv,
+k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, int Bpad, const T* __restrict__ dSinv,
          const T* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
          const T* __restrict__ GD, T* __restrict__ Wcat, long ldw) {
   __shared__ T p2s[PAWFE_MAX_NPJ][kCoupleLanes + 1];
   const int a = blockIdx.x;
   const int lane = threadIdx.x % kCoupleLanes, al = threadIdx.x / kCoupleLanes;   // al < npj
   const int v = blockIdx.y * kCoupleLanes + lane;
-  const bool ok = v < B;
+  const bool ok = v < B, wr = v < Bpad;   // wr && !ok: pad column, every product below is zero
   T p1[PAWFE_MAX_NPJ];
 #pragma unroll
   for (int be = 0; be < PAWFE_MAX_NPJ; ++be) p1[be] = (ok && be < npj) ? P1[((long)a * npj + be) * ldp + v] : s_zero(T());
@@ -283,8 +286,8 @@ k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, const T* 
     T s = s_zero(T());
 #pragma unroll
     for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[be], p1[be]);
-    if (ok) Wa[(long)al * ldw + v] = s;
-  } else if (ok) {
+    if (wr) Wa[(long)al * ldw + v] = s;
+  } else if (wr) {
     Wa[(long)al * ldw + v] = s_zero(T());
   }
   if (mode == 1) return;
@@ -306,7 +309,7 @@ k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, const T* 
   T w2 = s_zero(T());
 #pragma unroll
   for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(w2, Da[be], p2s[be][lane]);
-  if (ok) Wa[(long)(npj + al) * ldw + v] = w2;
+  if (wr) Wa[(long)(npj + al) * ldw + v] = w2;
 }
 
 // X[J][v] += scale * M_D^-1[J] * sum_al C^{e,a}[I][al] W^a[al][v] over the pairs (recovery: scale = -1).
@@ -367,169 +370,6 @@ __device__ inline double mdinv_row(const MeshDev& md, long J) {
   int iy = (int)(t % md.N[1]);
   int ix = (int)(t / md.N[1]);
   return md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
-}
-
-// Alg. 2 steps 2-3 (L260-L264) in the scaled variables:  Yt = M_D^-1 (HX - SX Lambda) (FP64, in place in HX);
-// Rt_Y = (zeta/e) Yt;  Rt_X = 0.  All arrays have leading dimension ldw; pad columns are written as 0.
-__global__ void k_residual_init2(MeshDev md, long ldw, int B, double* __restrict__ HX, const double* __restrict__ SX,
-                                 const double* __restrict__ lam, double z_over_e, float* __restrict__ RX,
-                                 float* __restrict__ RY) {
-  const long total = md.M * ldw;
-  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
-    const long J = idx / ldw;
-    const int v = (int)(idx - J * ldw);
-    double y = 0.0;
-    if (v < B) y = mdinv_row(md, J) * (HX[idx] - SX[idx] * lam[v]);
-    HX[idx] = y;
-    RY[idx] = (float)(z_over_e * y);
-    RX[idx] = 0.f;
-  }
-}
-
-// Bracket of Alg. 2 step 4 (L272) without the H term:  Rt_X <- (-a c) Rt_Y - (zeta zeta1) Rt_X  [FP32]
-//                                                           + Yt (a Lambda_Y)                  [FP64 add, L374]
-// 4 consecutive vectors per thread; ldw % 4 == 0.
-__global__ void __launch_bounds__(256)
-k_prepass(long nquads, int ldq /* ldw / 4 */, const float4* __restrict__ RY, float4* __restrict__ RX,
-          const double2* __restrict__ Yt, const double* __restrict__ aLamY, int B /*real columns*/, int cw, float ac, float zz1) {
-  for (long q = blockIdx.x * (long)blockDim.x + threadIdx.x; q < nquads; q += (long)gridDim.x * blockDim.x) {
-    const int v = (int)(q % ldq) * 4;
-    const float4 ry = RY[q];
-    const float4 rx = RX[q];
-    const double2 y0 = Yt[2 * q], y1 = Yt[2 * q + 1];
-    double l0 = 0, l1 = 0, l2 = 0, l3 = 0;
-    if (v < B) l0 = aLamY[v / cw];
-    if (v + 1 < B) l1 = aLamY[(v + 1) / cw];
-    if (v + 2 < B) l2 = aLamY[(v + 2) / cw];
-    if (v + 3 < B) l3 = aLamY[(v + 3) / cw];
-    float4 o;
-    o.x = (float)((double)(-ac * ry.x - zz1 * rx.x) + y0.x * l0);
-    o.y = (float)((double)(-ac * ry.y - zz1 * rx.y) + y0.y * l1);
-    o.z = (float)((double)(-ac * ry.z - zz1 * rx.z) + y1.x * l2);
-    o.w = (float)((double)(-ac * ry.w - zz1 * rx.w) + y1.y * l3);
-    RX[q] = o;
-  }
-}
-
-// Bracket of Alg. 2 step 4 (as k_prepass) and the projection P1 = C^T Rt_Y (as k_proj2) in ONE sweep over Rt_Y: a CTA is a
-// cell x 128 columns; it reads the cell's rows once, writes the bracket for the nodes the cell owns (every node has exactly
-// one owner cell) and accumulates the projection of the cell's first (cell, atom) pair on the rows it already holds;
-// further pairs of the cell re-read the rows (L1 / L2 hits).  The streaming part leaves the issue slots to the FMAs of
-// the projection, which as a kernel of its own was issue / latency-bound (profiles/r01_ncu_small_kernels.md).
-// Opt-in (PAWFE_PPFUSE=1): parity-green, but at 2 CTAs x 256 threads per SM and two rows in flight per thread it moves
-// 4.2 GB in 1.02 ms (4.1 TB/s) against 0.53 + 0.29 ms for k_prepass + k_proj2, so the separate kernels stay the default.
-//   grid = (ncell, ceil(ldw/128)), block = 256.  dynamic smem: n longs + NPJ*n floats + NPJ*128 floats + n bytes.
-//   P zero on entry.  Real contexts.  ldw % 4 == 0; P rows have ldp >= ldw.
-template <int NPJ>
-__global__ void __launch_bounds__(256, 2)
-k_prepass_proj(MeshDev md, const int* __restrict__ cps, const int* __restrict__ cpi, const int* __restrict__ pair_atom,
-               const float* __restrict__ Cd, const float* __restrict__ RY, float* __restrict__ RX,
-               const double* __restrict__ Yt, long ldw, int B, const double* __restrict__ aLamY, float ac, float zz1,
-               float* __restrict__ P, long ldp) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int n = md.n, n1 = md.n1, pp = md.p;
-  long* nodeJ = reinterpret_cast<long*>(smem_raw);                       // row index (always valid)
-  float* Cs = reinterpret_cast<float*>(nodeJ + (n + 1) / 2 * 2);         // [NPJ][n]
-  float* red = Cs + ((size_t)NPJ * n + 3) / 4 * 4;                       // [NPJ][128]
-  unsigned char* flag = reinterpret_cast<unsigned char*>(red + NPJ * 128);   // bit 0: owned by this cell, bit 1: masked
-  const int e = blockIdx.x;
-  const int q0 = cps[e], nq = cps[e + 1] - q0;
-  int cx, cy, cz;
-  mesh_cell_coords(md, e, &cx, &cy, &cz);
-  for (int I = threadIdx.x; I < n; I += blockDim.x) {
-    int c = I % n1, b = (I / n1) % n1, a = I / (n1 * n1), ix, iy, iz;
-    nodeJ[I] = mesh_node(md, cx, cy, cz, a, b, c, &ix, &iy, &iz);
-    const bool own = (a < pp || (!md.periodic && cx == md.nc[0] - 1)) && (b < pp || (!md.periodic && cy == md.nc[1] - 1)) &&
-                     (c < pp || (!md.periodic && cz == md.nc[2] - 1));
-    const bool masked = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0;
-    flag[I] = (own ? 1 : 0) | (masked ? 2 : 0);
-  }
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int v = blockIdx.y * 128 + lane * 4;
-  const bool vok = v < ldw;
-  double l0 = 0, l1 = 0, l2 = 0, l3 = 0;
-  if (v < B) l0 = aLamY[v];
-  if (v + 1 < B) l1 = aLamY[v + 1];
-  if (v + 2 < B) l2 = aLamY[v + 2];
-  if (v + 3 < B) l3 = aLamY[v + 3];
-  for (int q = 0; q < (nq > 0 ? nq : 1); ++q) {
-    const int pr = nq > 0 ? cpi[q0 + q] : -1;
-    __syncthreads();   // nodeJ / flag written (q = 0); everyone is done with Cs and red of the previous pair
-    if (pr >= 0) {
-      for (int i = threadIdx.x; i < NPJ * n; i += blockDim.x) Cs[i] = Cd[(long)pr * NPJ * n + i];
-      for (int i = threadIdx.x; i < NPJ * 128; i += blockDim.x) red[i] = 0.f;
-    }
-    __syncthreads();
-    float4 acc[NPJ];
-#pragma unroll
-    for (int al = 0; al < NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (vok) {
-      // rows w, w + 8, ...; two rows in flight per thread
-      for (int I0 = w; I0 < n; I0 += 16) {
-        float4 ry[2], rx[2];
-        double2 ya[2], yb[2];
-        int fl[2];
-        long off[2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          const int I = I0 + 8 * u;
-          fl[u] = I < n ? flag[I] : 2;
-          off[u] = I < n ? nodeJ[I] * ldw + v : 0;
-          const bool brk = I < n && q == 0 && (fl[u] & 1);
-          const bool prj = pr >= 0 && !(fl[u] & 2);
-          fl[u] = (brk ? 1 : 0) | (prj ? 2 : 0);
-          ry[u] = (brk || prj) ? __ldg(reinterpret_cast<const float4*>(RY + off[u])) : make_float4(0.f, 0.f, 0.f, 0.f);
-          if (brk) {
-            rx[u] = *reinterpret_cast<const float4*>(RX + off[u]);
-            ya[u] = __ldg(reinterpret_cast<const double2*>(Yt + off[u]));
-            yb[u] = __ldg(reinterpret_cast<const double2*>(Yt + off[u] + 2));
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          if (fl[u] & 1) {
-            float4 o;
-            o.x = (float)((double)(-ac * ry[u].x - zz1 * rx[u].x) + ya[u].x * l0);
-            o.y = (float)((double)(-ac * ry[u].y - zz1 * rx[u].y) + ya[u].y * l1);
-            o.z = (float)((double)(-ac * ry[u].z - zz1 * rx[u].z) + yb[u].x * l2);
-            o.w = (float)((double)(-ac * ry[u].w - zz1 * rx[u].w) + yb[u].y * l3);
-            *reinterpret_cast<float4*>(RX + off[u]) = o;
-          }
-          if (fl[u] & 2) {
-            const int I = I0 + 8 * u;
-#pragma unroll
-            for (int al = 0; al < NPJ; ++al) {
-              const float cv = Cs[al * n + I];
-              acc[al].x = fmaf(cv, ry[u].x, acc[al].x); acc[al].y = fmaf(cv, ry[u].y, acc[al].y);
-              acc[al].z = fmaf(cv, ry[u].z, acc[al].z); acc[al].w = fmaf(cv, ry[u].w, acc[al].w);
-            }
-          }
-        }
-      }
-    }
-    if (pr < 0) break;   // uniform: a cell without pairs only writes the bracket
-    for (int r = 0; r < 8; ++r) {   // ordered cross-warp sum
-      if (w == r && vok) {
-#pragma unroll
-        for (int al = 0; al < NPJ; ++al) {
-          float4* qd = reinterpret_cast<float4*>(red + al * 128 + lane * 4);
-          float4 t = *qd;
-          t.x += acc[al].x; t.y += acc[al].y; t.z += acc[al].z; t.w += acc[al].w;
-          *qd = t;
-        }
-      }
-      __syncthreads();
-    }
-    const int a = pair_atom[pr];
-    for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
-      const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
-      if (vv < ldw) {
-        const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
-        float* dst = P + ((long)a * NPJ + al) * ldp + vv;
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
-      }
-    }
-  }
 }
 
 // Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
@@ -697,10 +537,14 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   return PAWFE_OK;
 }
 
+// Scratch of the fused path for blocks of up to Bvec vectors: projections, couplings (and their low parts for the FP32
+// mode), FP64 projections of the residual set-up.  Grows on the first call and when a wider block arrives (stream
+// synchronisation + allocation: pawfe_prepare does this ahead of the hot calls).
 pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int Bvec) {
   const int B = Bvec * (c->cplx ? 2 : 1);   // real columns
   if (B <= p->Bcap) return PAWFE_OK;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (p->aux) CUDA_TRY(c, cudaStreamSynchronize(p->aux));
   cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64); cudaFree(p->d_Wcat_lo);
   p->d_Wcat_lo = nullptr;
   p->d_P1 = p->d_Wcat = nullptr; p->d_P64 = p->d_W64 = nullptr; p->Bcap = 0;
@@ -713,6 +557,16 @@ pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int Bvec) {
   TRY(dev_alloc(c, &p->d_W64, na * c->npj * ldw));
   CUDA_TRY(c, cudaMemsetAsync(p->d_Wcat, 0, na * 32 * ldw * sizeof(float), c->stream));
   p->Bcap = B; p->ldw = ldw;
+  return PAWFE_OK;
+}
+
+// a block-sized scratch array of the plan (low parts / scaled copy of an apply's input block)
+pawfe_status ensure_block(pawfe_ctx* c, FusedPlan* p, float** buf, size_t* have, size_t want) {
+  if (*have >= want) return PAWFE_OK;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  cudaFree(*buf); *buf = nullptr; *have = 0;
+  TRY(dev_alloc(c, buf, want));
+  *have = want;
   return PAWFE_OK;
 }
 
@@ -729,16 +583,9 @@ pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, 
 }
 
 // X: the block as floats (complex: interleaved), ldx in floats; B vectors.
-pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode, bool projected = false) {
+pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
-  if (projected) {   // P1 already holds C^T X (k_prepass_proj): couplings only
-    k_couple<float><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
-        npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
-        p->d_GD, p->d_Wcat, p->ldw);
-    KERNEL_CHECK(c, "k_couple");
-    return PAWFE_OK;
-  }
   CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
   if (c->cplx) {
     switch (npj) {
@@ -747,8 +594,9 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
       CASE_PC(9) CASE_PC(10) CASE_PC(11) CASE_PC(12) CASE_PC(13) CASE_PC(14) CASE_PC(15) CASE_PC(16)
 #undef CASE_PC
     }
-    k_couple<float2><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
-        npj, mode, (const float2*)p->d_P1, p->ldw / 2, B, (const float2*)c->d_dSinv32, (const float2*)c->d_D32, p->d_nb_start,
+    const int Bpad = (int)(roundup4(2 * B) / 2);
+    k_couple<float2><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
+        npj, mode, (const float2*)p->d_P1, p->ldw / 2, B, Bpad, (const float2*)c->d_dSinv32, (const float2*)c->d_D32, p->d_nb_start,
         p->d_nb_atom, (const float2*)p->d_GD, (float2*)p->d_Wcat, p->ldw / 2);
     KERNEL_CHECK(c, "k_couple");
     return PAWFE_OK;
@@ -770,8 +618,9 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   }
 #undef LAUNCH_PROJ2
   KERNEL_CHECK(c, "k_proj2");
-  k_couple<float><<<dim3(c->natoms, ceil_div(B, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
-      npj, mode, p->d_P1, p->ldw, B, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
+  const int Bpad = (int)roundup4(B);
+  k_couple<float><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
+      npj, mode, p->d_P1, p->ldw, B, Bpad, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
       p->d_GD, p->d_Wcat, p->ldw);
   KERNEL_CHECK(c, "k_couple");
   return PAWFE_OK;
@@ -815,6 +664,7 @@ TcExt make_ext(const FusedPlan* p, int scale_mode) {
   TcExt x;
   x.scale_mode = scale_mode; x.nchunks = p->nchunks; x.ext_start = p->d_ext_start; x.ext_atom = p->d_ext_atom;
   x.Bext = p->d_Bext; x.Wcat = p->d_Wcat; x.ldw = p->ldw; x.ksteps = p->ext_ksteps;
+  x.Hstream = nullptr;
   return x;
 }
 
@@ -828,7 +678,7 @@ bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
   return (prec == PAWFE_TF32 || (prec == PAWFE_FP32 && !c->cplx)) && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
 }
 
-// run `body` on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream
+// run work on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream
 #define FORK_AUX(c, p) do { if ((p)->no_aux) break; CUDA_TRY(c, cudaEventRecord((p)->ev_fork, (c)->stream)); CUDA_TRY(c, cudaStreamWaitEvent((p)->aux, (p)->ev_fork, 0)); } while (0)
 #define JOIN_AUX(c, p) do { if ((p)->no_aux) break; CUDA_TRY(c, cudaEventRecord((p)->ev_join, (p)->aux)); CUDA_TRY(c, cudaStreamWaitEvent((c)->stream, (p)->ev_join, 0)); } while (0)
 struct StreamSwap {   // kernels launched while this lives go to `s`
@@ -840,74 +690,113 @@ struct StreamSwap {   // kernels launched while this lives go to `s`
 pawfe_status fused_prepare(pawfe_ctx* c, int B) {
   FusedPlan* p = (FusedPlan*)c->fused;
   if (!p) {
+    TRY(tc_prepare(c));
     p = new FusedPlan();
     c->fused = p;
     // highest priority: the auxiliary kernels are short and latency-bound; their CTAs should take every slot that frees up
-    // next to the bandwidth-bound kernel of the main stream instead of queueing behind its whole grid
+    // next to the long kernel of the main stream instead of queueing behind its whole grid
     int prio_lo = 0, prio_hi = 0;
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
-    if (cudaStreamCreateWithPriority(&p->aux, cudaStreamNonBlocking, getenv("PAWFE_AUX_PRIO0") ? 0 : prio_hi) != cudaSuccess ||
+    if (cudaStreamCreateWithPriority(&p->aux, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
       cudaGetLastError(); fused_invalidate(c); c->err = "fused plan: stream / event creation failed"; return PAWFE_ECUDA;
     }
-    p->no_aux = getenv("PAWFE_NO_AUX") != nullptr;
-    p->ppfuse = getenv("PAWFE_PPFUSE") != nullptr;
+    p->no_aux = getenv("PAWFE_NO_AUX") != nullptr;   // read once, here: everything on the context's stream (timing experiments)
     pawfe_status st = build_plan(c, p);
     if (st != PAWFE_OK) { fused_invalidate(c); return st; }
   }
   return ensure_scratch(c, p, B);
 }
 
-// One cell-level pass  Y += alpha [M_D^-1] (H_loc X + K-extension terms).  TF32: one launch.  FP32 ("FP32"):
-// three launches with the operands split into the part the tensor core keeps (hi = trunc_tf32) and the rest (lo):
-//   hi x hi + lo x hi + hi x lo   (the dropped lo x lo term is ~2^-22 relative), FP32 accumulation throughout.
+// Everything the fused path allocates lazily, now: plan, scratch for blocks of up to B vectors, and for PAWFE_FP32 the low
+// parts of the operand streams and a block-sized scratch; with_block: the block-sized scratch of pawfe_apply_HSinv too.
+pawfe_status fused_prepare_all(pawfe_ctx* c, pawfe_prec prec, int B, bool with_block) {
+  TRY(fused_prepare(c, B));
+  FusedPlan* p = (FusedPlan*)c->fused;
+  const size_t blk = (size_t)c->M * roundup4((long)B * (c->cplx ? 2 : 1));
+  if (prec == PAWFE_FP32) {
+    const float* hlo = nullptr;
+    TRY(tc_hstream_lo(c, &hlo));
+    if (p->nchunks > 0 && !p->d_Bext_lo) {
+      int NH = 1, NT = c->n;
+      tc_shape(c, &NH, &NT);
+      const size_t cnt = (size_t)p->nchunks * NH * NT * 32 * (c->cplx ? 2 : 1);
+      TRY(dev_alloc(c, &p->d_Bext_lo, cnt));
+      TRY(tc_lo_part(c, p->d_Bext, p->d_Bext_lo, (long)cnt));
+    }
+    if (with_block) TRY(ensure_block(c, p, &p->d_xlo, &p->xlo_elems, blk));
+  }
+  if (with_block) TRY(ensure_block(c, p, &p->d_xs, &p->xs_elems, blk));
+  return PAWFE_OK;
+}
+
+// One cell-level pass: Y <- epi(alpha [M_D^-1] (H_loc X + K-extension terms)).  TF32: one launch.  FP32 (PAPER.md:L374
+// "FP32"): three launches with the operands split into the part the tensor core keeps (hi = trunc_tf32) and the rest (lo):
+//   hi x hi + lo x hi + hi x lo   (the dropped lo x lo term is ~2^-22 relative), FP32 accumulation throughout;
+// the first launch runs the caller's epilogue, the other two add to its result.
 // xlo: scratch for the low parts of X (same shape).  Wcat holds the couplings of this step.
 pawfe_status cell_pass(pawfe_ctx* c, FusedPlan* p, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B,
-                       float alpha, int scale_mode, float* xlo) {
+                       float alpha, int scale_mode, const TcEpi& epi, float* xlo) {
   TcExt x = make_ext(p, scale_mode);
-  x.Hstream = nullptr;
   prof_begin(c);
-  pawfe_status st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x);
+  pawfe_status st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x, &epi);
   if (st == PAWFE_OK && prec == PAWFE_FP32) {
     const float* hlo = nullptr;
     st = tc_hstream_lo(c, &hlo);
-    if (st == PAWFE_OK && p->nchunks > 0 && !p->d_Bext_lo) {
+    if (st == PAWFE_OK && p->nchunks > 0 && !p->d_Bext_lo) {   // first FP32-mode use without pawfe_prepare
       int NH = 1, NT = c->n;
       tc_shape(c, &NH, &NT);
-      const size_t cnt = (size_t)p->nchunks * NH * NT * 32;
+      const size_t cnt = (size_t)p->nchunks * NH * NT * 32 * (c->cplx ? 2 : 1);
       st = dev_alloc(c, &p->d_Bext_lo, cnt);
       if (st == PAWFE_OK) st = tc_lo_part(c, p->d_Bext, p->d_Bext_lo, (long)cnt);
     }
     if (st == PAWFE_OK) st = tc_lo_part(c, X, xlo, c->M * ldx);
     if (st == PAWFE_OK && c->natoms > 0) st = tc_lo_part(c, p->d_Wcat, p->d_Wcat_lo, (long)c->natoms * 32 * p->ldw);
+    TcEpi add; add.mode = TC_EPI_ADD; add.Yt = nullptr; add.aLam = nullptr; add.ac = add.zz1 = 0.f; add.cw = 1;
     if (st == PAWFE_OK) {           // lo(X) x hi(H)
       TcExt x2 = x; x2.Wcat = p->d_Wcat_lo;
-      st = tc_cell_apply(c, xlo, ldx, Y, ldy, B, alpha, &x2);
+      st = tc_cell_apply(c, xlo, ldx, Y, ldy, B, alpha, &x2, &add);
     }
     if (st == PAWFE_OK) {           // hi(X) x lo(H)
       TcExt x3 = x; x3.Bext = p->d_Bext_lo; x3.Hstream = hlo;
-      st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x3);
+      st = tc_cell_apply(c, X, ldx, Y, ldy, B, alpha, &x3, &add);
     }
   }
   prof_end(c);
   return st;
 }
 
+static TcEpi epi_plain(int mode) {
+  TcEpi e; e.mode = mode; e.Yt = nullptr; e.aLam = nullptr; e.ac = e.zz1 = 0.f; e.cw = 1;
+  return e;
+}
+
+// Y = H X: every row of Y is stored by its first writer (no zero-fill), the non-local term rides in the K-extension
 pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B) {
   TRY(fused_prepare(c, B));
   FusedPlan* p = (FusedPlan*)c->fused;
-  if (prec == PAWFE_FP32 && p->xlo_elems < (size_t)c->M * ldx) {
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    cudaFree(p->d_xlo); p->d_xlo = nullptr; p->xlo_elems = 0;
-    TRY(dev_alloc(c, &p->d_xlo, (size_t)c->M * ldx));
-    p->xlo_elems = (size_t)c->M * ldx;
-  }
+  if (prec == PAWFE_FP32) TRY(ensure_block(c, p, &p->d_xlo, &p->xlo_elems, (size_t)c->M * ldx));
   const int Wr = B * (c->cplx ? 2 : 1);   // X, Y as float blocks: ldx, ldy in floats, Wr real columns
   TRY(project_and_couple(c, p, X, ldx, B, 2));
-  if (ldy == Wr) CUDA_TRY(c, cudaMemsetAsync(Y, 0, (size_t)c->M * Wr * sizeof(float), c->stream));
-  else CUDA_TRY(c, cudaMemset2DAsync(Y, ldy * sizeof(float), 0, (size_t)Wr * sizeof(float), c->M, c->stream));
-  return cell_pass(c, p, prec, X, ldx, Y, ldy, Wr, 1.0f, 0, p->d_xlo);
+  return cell_pass(c, p, prec, X, ldx, Y, ldy, Wr, 1.0f, 0, epi_plain(TC_EPI_STORE), p->d_xlo);
+}
+
+// Y = H S^-1approx X (the operator the filter iterates, Alg. 1 step 2 L244 / Eq. 30) in exactly the kernel
+// configuration of the filter's step: Xs = M_D^-1 X, P1 = C^T Xs, couplings W / W2, one cell pass with both halves of
+// the K-extension.  X, Y as float blocks (complex: interleaved; ldx, ldy in floats).
+pawfe_status fused_apply_HSinv(pawfe_ctx* c, pawfe_prec prec, const float* X, long ldx, float* Y, long ldy, int B) {
+  TRY(fused_prepare(c, B));
+  FusedPlan* p = (FusedPlan*)c->fused;
+  const int Wr = B * (c->cplx ? 2 : 1);
+  const long lds = roundup4(Wr);
+  TRY(ensure_block(c, p, &p->d_xs, &p->xs_elems, (size_t)c->M * lds));
+  if (prec == PAWFE_FP32) TRY(ensure_block(c, p, &p->d_xlo, &p->xlo_elems, (size_t)c->M * lds));
+  if (lds != Wr) CUDA_TRY(c, cudaMemsetAsync(p->d_xs, 0, (size_t)c->M * lds * sizeof(float), c->stream));   // pad columns
+  k_scale_mdinv_f4<<<8 * c->sm_count, 256, 0, c->stream>>>(c->md, (const float4*)X, ldx / 4, (float4*)p->d_xs, lds / 4, Wr / 4);
+  KERNEL_CHECK(c, "k_scale_mdinv_f4");
+  TRY(project_and_couple(c, p, p->d_xs, lds, B, 0));
+  return cell_pass(c, p, prec, p->d_xs, lds, Y, ldy, Wr, 1.0f, 0, epi_plain(TC_EPI_STORE), p->d_xlo);
 }
 
 // recovery's low-rank part for complex contexts:  X -= M_D^-1 C W  (W = rows [0, npj) of Wcat)
@@ -922,34 +811,40 @@ static pawfe_status scatter_cplx(pawfe_ctx* c, FusedPlan* p, float* X, long ldx,
   return PAWFE_OK;
 }
 
-pawfe_status launch_prepass_proj(pawfe_ctx* c, FusedPlan* p, const float* RY, float* RX, const double* Yt, long ldw, int B,
-                                 const double* aLamY, float ac, float zz1) {
-  const int n = c->n, npj = c->npj;
-  const size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4 + (size_t)(n + 15) / 16 * 16;
-  dim3 grid((unsigned)c->ncell, ceil_div((int)ldw, 128));
-#define LAUNCH_PP(NPJ)                                                                                               \
-  do {                                                                                                               \
-    TRY(pawfe_ensure_smem(c, (const void*)k_prepass_proj<NPJ>, smem));                                               \
-    k_prepass_proj<NPJ><<<grid, 256, smem, c->stream>>>(c->md, p->d_cps, p->d_cpi, c->d_pair_atom, (const float*)c->d_Cd32, RY, RX, \
-                                                        Yt, ldw, B, aLamY, ac, zz1, p->d_P1, p->ldw);                  \
-  } while (0)
-  switch (npj) {
-    case 1: LAUNCH_PP(1); break;   case 2: LAUNCH_PP(2); break;   case 3: LAUNCH_PP(3); break;
-    case 4: LAUNCH_PP(4); break;   case 5: LAUNCH_PP(5); break;   case 6: LAUNCH_PP(6); break;
-    case 7: LAUNCH_PP(7); break;   case 8: LAUNCH_PP(8); break;   case 9: LAUNCH_PP(9); break;
-    case 10: LAUNCH_PP(10); break; case 11: LAUNCH_PP(11); break; case 12: LAUNCH_PP(12); break;
-    case 13: LAUNCH_PP(13); break; case 14: LAUNCH_PP(14); break; case 15: LAUNCH_PP(15); break;
-    default: LAUNCH_PP(16); break;
+// Step 2 of Alg. 2 for real contexts (L260, L374), FP64, S X never stored:  Yt <- H X - S X Lambda  (unscaled; the caller
+// scales).  The DMMA product runs on the context's stream, the mass sweeps and the FP64 non-local part (both add into Yt
+// with FP64 atomics) on the auxiliary stream; on any failure the auxiliary stream is joined before returning.
+static pawfe_status residual_setup_real(pawfe_ctx* c, FusedPlan* p, const float* X, long ld, int B, double* Yt, long ldw,
+                                        const double* lam, const double* neg_lam) {
+  CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
+  FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
+  pawfe_status st = pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B);
+  {
+    StreamSwap sw(c, p->no_aux ? c->stream : p->aux);
+    if (st == PAWFE_OK) {
+      const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
+      st = pawfe_ensure_smem(c, (const void*)k_mass_sf<float, kMassCT>, smem);
+      if (st == PAWFE_OK) {
+        k_mass_sf<float, kMassCT><<<dim3(c->ncell, ceil_div(B, kMassCT)), 256, smem, c->stream>>>(
+            c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, neg_lam);
+        c->launches++;
+        if (cudaGetLastError() != cudaSuccess) { c->err = "k_mass_sf launch failed"; st = PAWFE_ECUDA; }
+      }
+    }
+    if (st == PAWFE_OK && c->npairs > 0) st = setup_nonlocal64(c, p, X, ld, B, lam, Yt, ldw);
   }
-#undef LAUNCH_PP
-  KERNEL_CHECK(c, "k_prepass_proj");
+  if (st != PAWFE_OK) { if (!p->no_aux) cudaStreamSynchronize(p->aux); return st; }
+  JOIN_AUX(c, p);
   return PAWFE_OK;
 }
 
 // X: the block in the context's FP32 storage scalar (float, or float2 interleaved), ld and B in those scalars.  Inside, every
 // array is a real block of Wr = B * cw columns (cw = 2 for complex contexts) with leading dimension ldw = roundup4(Wr).
+// HX, SX: null (step 2 computed here, L260) or the caller's FP64 blocks H X and S X in X's layout (leading dimension ld,
+// FP64 scalars): step 2 is then Y = HX - SX Lambda without any operator application (pawfe_cheb_filter_hs).
 pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds, const double* as, const double* acs,
-                          const double* zzs, double z_over_e, void* Xv, long ld, int B, void* workspace) {
+                          const double* zzs, double z_over_e, void* Xv, long ld, int B, void* workspace,
+                          const void* HX, const void* SX) {
   TRY(fused_prepare(c, B));
   FusedPlan* p = (FusedPlan*)c->fused;
   const int cw = c->cplx ? 2 : 1;
@@ -964,55 +859,31 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   float* RX = (float*)(ws + blk_d);
   float* RY = (float*)(ws + blk_d + blk_s);
   float* XLO = (float*)(ws + blk_d + 2 * blk_s);   // FP32 mode only (pawfe_filter_workspace adds the block)
-  // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda; S X is never stored ----
-  if (c->cplx) {
+  const int gs = 8 * c->sm_count;
+  const double* lam = ds;
+  const double* neg_lam = ds + (size_t)(m + 1) * B;
+  // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda ----
+  if (HX && SX) {
+    k_residual_from_products<<<gs, 256, 0, c->stream>>>(c->M, ldw, Wr, cw, (const double*)HX, (const double*)SX, ldx, lam, Yt);
+    KERNEL_CHECK(c, "k_residual_from_products");
+  } else if (c->cplx) {
     // complex: the generic FP64 applies (DMMA cell product, mass sweeps, Ritz values folded into the coupling)
     TRY((pawfe_apply_HS<float2, double2, double2>(c, 0, false, (const float2*)X, ld, (double2*)Yt, ldw / 2, B)));
-    TRY((pawfe_sub_SX_lambda<float2, double2>(c, (const float2*)X, ld, (double2*)Yt, ldw / 2, B, ds, ds + (size_t)(m + 1) * B)));
+    TRY((pawfe_sub_SX_lambda<float2, double2>(c, (const float2*)X, ld, (double2*)Yt, ldw / 2, B, lam, neg_lam)));
   } else {
-    // real: fused (setup_fp64.cuh)
-    CUDA_TRY(c, cudaMemsetAsync(Yt, 0, (size_t)c->M * ldw * sizeof(double), c->stream));
-    FORK_AUX(c, p);                                                 // Yt is zero from here on for both streams
-    bool mass_done = false;                                         // DMMA-bound, on the main stream; p <= 6: mass term inside
-    TRY(pawfe_cell_product_fp64_mass(c, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B, &mass_done));
-    if (!mass_done) TRY(pawfe_cell_product_fp64<float>(c, X, ld, Yt, ldw, B));
-    {
-      StreamSwap sw(c, p->no_aux ? c->stream : p->aux);                                     // mass sweeps and non-local part: atomics into Yt, concurrently
-      if (!mass_done) {
-        const size_t smem = (size_t)c->n * kMassCT * 8 + (size_t)c->n * 8;
-        TRY(pawfe_ensure_smem(c, (const void*)k_mass_sf<float, kMassCT>, smem));
-        k_mass_sf<float, kMassCT><<<dim3(c->ncell, ceil_div(B, kMassCT)), 256, smem, c->stream>>>(
-            c->md, c->d_M1, c->h[0] * c->h[1] * c->h[2] / 8.0, X, ld, Yt, ldw, B, ds + (size_t)(m + 1) * B);
-        KERNEL_CHECK(c, "k_mass_sf");
-      }
-      if (c->npairs > 0) TRY(setup_nonlocal64(c, p, X, ld, B, ds, Yt, ldw));
-    }
-    JOIN_AUX(c, p);
+    TRY(residual_setup_real(c, p, X, ld, B, Yt, ldw, lam, neg_lam));
   }
-  const int gs = 8 * c->sm_count;
-  int gs_pre = gs;   // timing experiments: fewer resident prepass CTAs leave room for the aux stream's projection CTAs
-  { const char* d = getenv("PAWFE_PREPASS_CPS"); if (d && atoi(d) >= 1) gs_pre = atoi(d) * c->sm_count; }
+  // ---- step 3 in the scaled variables: Yt = M_D^-1 Y, Rt_Y = (zeta/e) Yt, Rt_X = 0 (pad columns 0) ----
   k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
-  // ---- step 4 ----
-  const long nquads = c->M * (ldw / 4);
-  const bool ppfuse = !c->cplx && c->npairs > 0 && p->d_cps && p->ppfuse;
+  // ---- step 4: one projection + coupling pass and ONE cell kernel per step; the cell kernel's first writers store the
+  //      bracket  -a c Rt_Y - zeta zeta1 Rt_X [FP32] + Yt (a Lambda_Y) [FP64 add, L374]  plus their own share of
+  //      a M_D^-1 H T, the other cells add theirs in cell order ----
   for (int th = 2; th <= m; ++th) {
-    if (ppfuse) {   // bracket and projection in one sweep over Rt_Y, then the couplings
-      CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * c->npj * p->ldw * sizeof(float), c->stream));
-      TRY(launch_prepass_proj(c, p, RY, RX, Yt, ldw, Wr, ds + (size_t)(th - 1) * B, (float)acs[th], (float)zzs[th]));
-      TRY(project_and_couple(c, p, RY, ldw, B, 0, true));
-      TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, XLO));
-      std::swap(RX, RY);
-      continue;
-    }
-    FORK_AUX(c, p);
-    { StreamSwap sw(c, p->no_aux ? c->stream : p->aux); TRY(project_and_couple(c, p, RY, ldw, B, 0)); }   // latency-bound, under the prepass
-    k_prepass<<<gs_pre, 256, 0, c->stream>>>(nquads, (int)(ldw / 4), (const float4*)RY, (float4*)RX, (const double2*)Yt,
-                                         ds + (size_t)(th - 1) * B, Wr, cw, (float)acs[th], (float)zzs[th]);
-    KERNEL_CHECK(c, "k_prepass");
-    JOIN_AUX(c, p);
-    TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, XLO));
+    TRY(project_and_couple(c, p, RY, ldw, B, 0));
+    TcEpi epi;
+    epi.mode = TC_EPI_BRACKET; epi.Yt = Yt; epi.aLam = ds + (size_t)(th - 1) * B; epi.ac = (float)acs[th]; epi.zz1 = (float)zzs[th]; epi.cw = cw;
+    TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, epi, XLO));
     std::swap(RX, RY);
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----

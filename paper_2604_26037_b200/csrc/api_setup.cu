@@ -93,6 +93,47 @@ extern "C" pawfe_status pawfe_local_potential_gaussians(pawfe_ctx* c, int natoms
   return PAWFE_OK;
 }
 
+namespace {
+// FP32 copy of the FP64 cell matrices with the padded row stride ldk (columns >= n are zero): [cell][n][ldk] scalars
+__global__ void k_h64_to_h32(const double* __restrict__ H64, int n, int ldk, int cw, long rows, float* __restrict__ H32) {
+  const long total = rows * ldk * cw;
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+    const int q = (int)(i % cw);
+    const long t = i / cw;
+    const int k = (int)(t % ldk);
+    const long row = t / ldk;                      // cell * n + I
+    H32[i] = k < n ? (float)H64[(row * n + k) * cw + q] : 0.f;
+  }
+}
+}  // namespace
+
+// User- (or oracle-) built cell matrices instead of pawfe_local_potential_gaussians.
+extern "C" pawfe_status pawfe_set_cell_matrices(pawfe_ctx* c, const double* Hcell, int is_device, int keep_fp64) {
+  if (!c || !Hcell) return PAWFE_EINVAL;
+  if (!c->have_mesh) { c->err = "mesh not created"; return PAWFE_ESTATE; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  pawfe_free_pot(c);
+  const int n = c->n, cw = c->cplx ? 2 : 1;
+  const size_t e64 = (size_t)c->ncell * n * n * cw, e32 = (size_t)c->ncell * n * c->ldk * cw;
+  double* H64 = nullptr; float* H32 = nullptr;
+  TRY(dev_alloc(c, &H64, e64));
+  c->d_H64 = H64;
+  cudaError_t e = cudaMemcpyAsync(H64, Hcell, e64 * sizeof(double), is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream);
+  if (e != cudaSuccess) { c->err = std::string("pawfe_set_cell_matrices copy: ") + cudaGetErrorString(e); pawfe_free_pot(c); return PAWFE_ECUDA; }
+  pawfe_status st = dev_alloc(c, &H32, e32);
+  if (st != PAWFE_OK) { pawfe_free_pot(c); return st; }
+  c->d_H32 = H32;
+  k_h64_to_h32<<<8 * c->sm_count, 256, 0, c->stream>>>(H64, n, c->ldk, cw, (long)c->ncell * n, H32);
+  c->launches++;
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { c->err = std::string("pawfe_set_cell_matrices: ") + cudaGetErrorString(e); pawfe_free_pot(c); return PAWFE_ECUDA; }
+  if (!keep_fp64) { cudaFree(c->d_H64); c->d_H64 = nullptr; }
+  c->have_pot = true;
+  c->have_h64 = keep_fp64 != 0;
+  return PAWFE_OK;
+}
+
 extern "C" pawfe_status pawfe_get_cell_matrix(pawfe_ctx* c, long cell, double* out) {
   if (!c || !out) return PAWFE_EINVAL;
   if (!c->have_pot || !c->have_h64) { c->err = "FP64 cell matrices not kept"; return PAWFE_ESTATE; }

@@ -20,5 +20,3 @@ pawfe_status pawfe_apply_H_any(pawfe_ctx* c, pawfe_prec prec, const void* X, lon
 // Y += sum_e P_e^T H^e (P_e X) in FP64 on the DMMA pipe, real contexts (no zeroing of Y, no non-local term).
 template <typename RX>
 pawfe_status pawfe_cell_product_fp64(pawfe_ctx* c, const RX* X, long ldx, double* Y, long ldy, int B);
-pawfe_status pawfe_cell_product_fp64_mass(pawfe_ctx* c, const float* X, long ldx, double* Y, long ldy, int B,
-                                          const double* neg_lam, bool* done);

@@ -50,8 +50,7 @@ __device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, uint32_
 template <typename RX, bool CPLX, int MT>
 __global__ void __launch_bounds__(kThreads, (MT <= 6 ? 2 : 1))
 k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const RX* __restrict__ X, long ldx,
-            double* __restrict__ Y, long ldy, int Wr, double alpha,
-            const double* __restrict__ M1 = nullptr, double mscale = 0.0, const double* __restrict__ mcoef = nullptr) {
+            double* __restrict__ Y, long ldy, int Wr, double alpha) {
   constexpr int KC = Cfg<CPLX>::KC, strideA = Cfg<CPLX>::strideA, cw = CPLX ? 2 : 1;
   constexpr int RB = 32 * MT;                       // rows per row block
   constexpr int strideB = sizeof(RX) == 4 ? kStrideB32 : kStrideB64;
@@ -88,55 +87,6 @@ k_cell_dmma(MeshDev md, const double* __restrict__ Amat, long cell_stride, const
     for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
       for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-
-    // Optional mass term (real blocks, one row block; the host checks that n x 64 doubles fit in the ring):
-    //   Y += alpha (A^e X_e + mcoef[v] mscale (M1 (x) M1 (x) M1) X_e)   -- residual set-up: A = H^e, mcoef = -Lambda,
-    // sum-factorised in the ring's shared memory BEFORE the first chunk and handed to the DMMAs as the accumulators'
-    // initial values, so the mass part costs no assembly atomics and no pass of its own (setup_fp64.cuh: k_mass_sf).
-    if (!CPLX && mcoef != nullptr) {
-      __shared__ double m1s[PAWFE_MAX_N1 * PAWFE_MAX_N1];
-      double* U = reinterpret_cast<double*>(stage0);   // [n][kTN]
-      const int n2 = n1 * n1;
-      for (int i = threadIdx.x; i < n2; i += kThreads) m1s[i] = M1[i];
-#pragma unroll 4
-      for (int i = threadIdx.x; i < n * kTN; i += kThreads) {
-        const int I = i / kTN, col = i % kTN;
-        const long J = nodeJ[I];
-        U[i] = (J >= 0 && v0 + col < Wr) ? (double)X[J * ldx + v0 + col] : 0.0;
-      }
-      __syncthreads();
-      for (int d = 2; d >= 0; --d) {   // three 1-D sweeps, direction d has stride n1^(2-d)
-        const int stride = d == 2 ? 1 : (d == 1 ? n1 : n2);
-        for (int i = threadIdx.x; i < n2 * kTN; i += kThreads) {
-          const int col = i % kTN, line = i / kTN;
-          const int q0 = line / n1, q1 = line % n1;
-          const int base = d == 2 ? (q0 * n1 + q1) * n1 : (d == 1 ? q0 * n2 + q1 : q0 * n1 + q1);
-          double t[PAWFE_MAX_N1];
-#pragma unroll
-          for (int k = 0; k < PAWFE_MAX_N1; ++k) t[k] = k < n1 ? U[(base + k * stride) * kTN + col] : 0.0;
-#pragma unroll
-          for (int r = 0; r < PAWFE_MAX_N1; ++r)
-            if (r < n1) {
-              double sacc = 0.0;
-#pragma unroll
-              for (int k = 0; k < PAWFE_MAX_N1; ++k) if (k < n1) sacc = fma(m1s[r * n1 + k], t[k], sacc);
-              U[(base + r * stride) * kTN + col] = sacc;
-            }
-        }
-        __syncthreads();
-      }
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt) {
-        const int I = (mt * 4 + rg) * 8 + (lane >> 2);
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-          const int col = vh * 32 + nt * 8 + 2 * (lane & 3);
-          if (I < n && v0 + col < Wr) acc[mt][nt][0] = mcoef[v0 + col] * mscale * U[I * kTN + col];
-          if (I < n && v0 + col + 1 < Wr) acc[mt][nt][1] = mcoef[v0 + col + 1] * mscale * U[I * kTN + col + 1];
-        }
-      }
-      __syncthreads();   // U is consumed before the ring overwrites it
-    }
 
     constexpr int RPP = kThreads / KC, NJ = RB / RPP;   // rows per sweep of the CTA, sweeps per chunk
     static_assert(RB % RPP == 0, "row block must be a multiple of the rows per sweep");

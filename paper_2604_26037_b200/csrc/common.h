@@ -188,6 +188,8 @@ struct pawfe_ctx {
   std::vector<cudaEvent_t> prof_ev;  // pairs (start, stop)
   size_t prof_used = 0;
 
+  void* d_tmpblk = nullptr; size_t tmpblk_bytes = 0;   // block T of the unfused pawfe_apply_HSinv
+
   // host-buffer filter (pawfe_cheb_filter_host)
   void* d_hostblk = nullptr; size_t hostblk_bytes = 0;
   void* d_hostws = nullptr;  size_t hostws_bytes = 0;

@@ -16,9 +16,10 @@ using namespace pawfe;
 
 pawfe_status pawfe_ensure_smem(pawfe_ctx* c, const void* func, size_t bytes) {
   static std::mutex mu;
-  static std::map<const void*, size_t> limit;   // per kernel: the limit set so far (default 48 KB needs no call)
+  // per (device, kernel): the limit set so far (default 48 KB needs no call); cudaFuncSetAttribute acts on the current device
+  static std::map<std::pair<int, const void*>, size_t> limit;
   std::lock_guard<std::mutex> lock(mu);
-  size_t& cur = limit[func];
+  size_t& cur = limit[std::make_pair(c->device, func)];
   if (bytes <= cur || bytes <= 48 * 1024) return PAWFE_OK;
   CUDA_TRY(c, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
   cur = bytes;
@@ -91,7 +92,7 @@ extern "C" pawfe_status pawfe_destroy(pawfe_ctx* c) {
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   cudaFree(c->d_scal);
   for (int i = 0; i < pawfe_ctx::kScalSlots; ++i) if (c->scal_ev[i]) cudaEventDestroy(c->scal_ev[i]);
-  cudaFree(c->d_hostblk); cudaFree(c->d_hostws); cudaFree(c->d_hostblk2);
+  cudaFree(c->d_hostblk); cudaFree(c->d_hostws); cudaFree(c->d_hostblk2); cudaFree(c->d_tmpblk);
   if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
   if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
   for (int i = 0; i < 2; ++i) {

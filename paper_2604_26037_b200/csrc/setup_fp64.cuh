@@ -226,3 +226,17 @@ k_residual_init3(MeshDev md, long ldw, int B, double* __restrict__ Y, double z_o
     reinterpret_cast<float4*>(RX)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
 }
+
+// Alg. 2 step 2 (L260) from products the caller already holds (pawfe_cheb_filter_hs: H Psi and S Psi of the last
+// Rayleigh-Ritz, rotated with the Ritz vectors, L402-L408):  Y = HX - SX Lambda, FP64.  HX, SX: [dof][ldx] doubles (complex:
+// interleaved, cw = 2 reals per vector); Y: [dof][ldw]; columns >= W of Y are left to k_residual_init3 (written as 0 there).
+static __global__ void __launch_bounds__(256)
+k_residual_from_products(long M, long ldw, int W, int cw, const double* __restrict__ HX, const double* __restrict__ SX,
+                         long ldx, const double* __restrict__ lam, double* __restrict__ Y) {
+  const long total = M * (long)W;
+  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+    const long J = idx / W;
+    const int v = (int)(idx - J * W);
+    Y[J * ldw + v] = HX[J * ldx + v] - SX[J * ldx + v] * lam[v / cw];
+  }
+}

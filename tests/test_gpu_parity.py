@@ -302,7 +302,7 @@ def test_filter_complex_odd_width_generic_sequence():
     want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
     Xd = _to_dev(X, "tf32", True)
     nbytes = ctx.filter_workspace(TF32, B)
-    assert nbytes > ctx.filter_workspace(TF32, B + 1)
+    assert nbytes >= ctx.filter_workspace(TF32, B + 1)      # complex contexts are always told the unfused sequence's size
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
@@ -342,32 +342,6 @@ def test_filter_host_block_set(name, prec):
         torch.cuda.synchronize()
         # same kernels on the same data: equal up to the order of the FP32 assembly reductions (R20)
         assert _relerr(_to_host(dev[k], cfg.complex), got) < (1e-12 if prec == "fp64" else 1e-5)
-
-
-@pytest.mark.parametrize("name", ["cfg1_twin", "cfg4_twin"])
-def test_filter_fused_prepass_projection_variant(name, monkeypatch):
-    """PAWFE_PPFUSE=1: bracket and projection in one sweep over Rt_Y (k_prepass_proj; every node's bracket is written by
-    the one cell that owns it: periodic and Dirichlet ownership rules) against the oracle's filter."""
-    from oracle import chfsi
-    from oracle.operators import PawOperators
-    from paper_2604_26037_b200 import TF32, context_from_system
-    monkeypatch.setenv("PAWFE_PPFUSE", "1")
-    cfg = _cases()[name]
-    sysd = make_system(cfg)
-    ops = PawOperators(sysd)
-    ctx = context_from_system(sysd, device=0, stream=torch.cuda.current_stream().cuda_stream)   # fresh plan reads the switch
-    B, m = 136, 5
-    X0 = random_block(cfg, B, stream=31) * ops.mask[:, None]
-    X = chfsi.s_orthonormalise(ops.apply_S, X0)
-    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
-    b0, bW, bU = _bounds(ops, lam)
-    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
-    Xd = _to_dev(X, "tf32", False)
-    nbytes = ctx.filter_workspace(TF32, B)
-    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
-    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
-    torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, False), want) < 5e-2
 
 
 # ---- degenerate and extreme cases --------------------------------------------------------------------------------
@@ -475,26 +449,6 @@ def test_error_behaviour():
     with pytest.raises(PawfeError, match="ESTATE"):
         bare.apply_H(TF32, X, Y, B, B)                                              # no potential, no atoms yet
     bare.destroy()
-
-
-def test_filter_mass_term_inside_fp64_cell_kernel(monkeypatch):
-    """PAWFE_MASSFOLD=1: the mass part of Y = H X - S X Lambda as the DMMA accumulators' initial values (cell_dmma.cuh)."""
-    from oracle import chfsi
-    from paper_2604_26037_b200 import TF32
-    monkeypatch.setenv("PAWFE_MASSFOLD", "1")
-    cfg, sysd, ops, ctx = _setup("cfg1_twin")
-    B, m = 72, 1    # m = 1: the result is the FP64 residual set-up alone, so a mass-term error is not hidden by TF32 noise
-    X0 = random_block(cfg, B, stream=61) * ops.mask[:, None]
-    X = chfsi.s_orthonormalise(ops.apply_S, X0)
-    X, lam = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
-    b0, bW, bU = _bounds(ops, lam)
-    want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
-    Xd = _to_dev(X, "tf32", False)
-    nbytes = ctx.filter_workspace(TF32, B)
-    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
-    ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
-    torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, False), want) < 5e-5
 
 
 @pytest.mark.parametrize("prec", ["fp64", "fp32", "tf32"])
