@@ -152,6 +152,17 @@ pawfe_status pawfe_apply_Sinv(pawfe_ctx* ctx, pawfe_prec prec, const void* X, vo
  * sequence of one filter step (projection, couplings, one cell contraction with the low-rank terms inside). */
 pawfe_status pawfe_apply_HSinv(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
 
+/* Y = S^-1approx X without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving
+ * loops, harnesses that forbid it).  Same result as pawfe_apply_Sinv up to the order of floating-point sums; same arguments.
+ * The projections and couplings (2 * natoms * nproj * B scalars of the precision mode's type; complex contexts: pairs)
+ * live in a static device array of 1 MiB (1,048,576 bytes) that every GPU that loads the library holds until the process
+ * exits; a block that needs more gives PAWFE_EINVAL with the sizes in pawfe_last_error (narrow B, or use pawfe_apply_Sinv).
+ * The call does no cudaMalloc / cudaFree and calls no allocating library routine; its FIRST call on a device looks the
+ * array's address up (cudaGetSymbolAddress, no allocation): make that call once outside graph capture.
+ * All calls on a device share the array and it keeps the last call's contents (the part in use is cleared first):
+ * calls that overlap on the GPU (other streams, other contexts on the same device) race on it. */
+pawfe_status pawfe_apply_Sinv_noalloc(pawfe_ctx* ctx, pawfe_prec prec, const void* X, void* Y, long ld, int B);
+
 /* Build every internal plan and scratch array the hot calls need for blocks of up to Bmax vectors, Chebyshev degree up to
  * mmax, in precision mode prec (see Conventions).  Optional; synchronises the host.  Call again after the operators
  * change or for a wider block. */

@@ -28,7 +28,7 @@ SYMBOLS = [
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
-    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs",
+    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc",
 ]
 
 
@@ -69,7 +69,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_prepare.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     lib.pawfe_cheb_filter_hs.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp, dp,
                                          C.c_long, C.c_int, vp, C.c_size_t]
-    for f in (lib.pawfe_apply_H, lib.pawfe_apply_S, lib.pawfe_apply_Sinv, lib.pawfe_apply_HSinv):
+    for f in (lib.pawfe_apply_H, lib.pawfe_apply_S, lib.pawfe_apply_Sinv, lib.pawfe_apply_HSinv, lib.pawfe_apply_Sinv_noalloc):
         f.argtypes = [vp, C.c_int, vp, vp, C.c_long, C.c_int]
     lib.pawfe_filter_workspace.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_size_t)]
     lib.pawfe_cheb_filter.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, dp,
@@ -238,6 +238,11 @@ class Context:
 
     def apply_Sinv(self, prec: int, X, Y, ld: int, B: int):
         self._check(self.lib.pawfe_apply_Sinv(self._h, int(prec), self._ptr(X), self._ptr(Y), int(ld), int(B)), "pawfe_apply_Sinv")
+
+    def apply_Sinv_noalloc(self, prec: int, X, Y, ld: int, B: int):
+        """S^-1approx X with its scratch in the library's static 1 MiB device array (no allocation; include/pawfe.h)."""
+        self._check(self.lib.pawfe_apply_Sinv_noalloc(self._h, int(prec), self._ptr(X), self._ptr(Y), int(ld), int(B)),
+                    "pawfe_apply_Sinv_noalloc")
 
     def apply_HSinv(self, prec: int, X, Y, ld: int, B: int):
         self._check(self.lib.pawfe_apply_HSinv(self._h, int(prec), self._ptr(X), self._ptr(Y), int(ld), int(B)), "pawfe_apply_HSinv")
