@@ -2,11 +2,16 @@
 """bench.py -- R-ChFSI filter throughput (dof x vector x Chebyshev-step per second) on B200.
 
 One "step" = one pass of the whole hot path (Algorithm 2: FP64 residual set-up, (m-1) x
-[S^-1approx, cell contraction + assembly, recurrence], recovery) over all N/B vector blocks of the
-workload = one "SCF-equivalent pass".  Workload at N=1: BASELINE.json configs[1] (16^3 cells, p=6,
-884,736 dofs, 400 vectors in blocks of 200, degree 20), synthetic seeded inputs.
+[projection + couplings, fused cell kernel = S^-1approx, cell contraction, ordered assembly, recurrence bracket], recovery)
+over all N/B vector blocks of the workload = one "SCF-equivalent pass".
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 1] [--prec tf32]
+Workload at N=1: the LARGEST single-GPU configuration of BASELINE.json, configs[4] (32^3 cells, p=6, Dirichlet, 7.19M stored
+dofs, 5,000 vectors in blocks of 256, degree 30).  Its 5,000 FP32 vectors (144 GB) do not fit beside the operators (47 GB)
+and the workspace, so a pass cycles through the distinct blocks that do fit (config.resident_blocks) and every timed call
+filters a fresh device copy of a block (7.4 GB >> L2).  `--config 1|2|3` run the other configs (all blocks resident where
+they fit), `--all-configs` prints one line per config 1-4.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 4] [--prec tf32]
 
 Multi-GPU: the path does not shard in this build ("replicas only"): under torchrun every rank
 filters its own replica of the workload on its own GPU; value = all ranks' units / max-over-ranks time.
@@ -77,6 +82,13 @@ def _cores_used() -> int:
     return 1
 
 
+def _host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -95,7 +107,8 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "sample": smp.desc},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": _cores_used(), "kind": "oracle", "sample": smp.desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": _cores_used(), "host_cores": _host_cores(), "kind": "oracle",
+                         "sample": smp.desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -196,18 +209,28 @@ def run_own(args):
     t_setup = time.perf_counter() - t_setup
     M, N, B, m = ctx.num_dofs(), cfg.nvec, cfg.block, cfg.degree
     cplx = cfg.complex
+    cw = 2 if cplx else 1
     hz = Harness(ctx, M, cplx)
     shape = (M, B, 2) if cplx else (M, B)
     nblk = (N + B - 1) // B
+    widths = [min(B, N - b * B) for b in range(nblk)]     # the last block of config 4 has 136 vectors
+    # plans, scratch and operand streams of the hot calls are built here, not inside the timed region (pawfe_prepare)
+    ctx.prepare(prec, B, m)
+    nbytes = ctx.filter_workspace(prec, B)
+    tdt = torch.float64 if prec == FP64 else torch.float32
+    es = (8 if prec == FP64 else 4) * cw
+    blk_bytes = M * B * es
+    # How many DISTINCT blocks stay resident.  All of them where they fit (configs 1-3); otherwise (config 4) as many as
+    # leave room for the workspace, a scratch block and the FP64 temporaries of the input preparation below.
+    free_b, _tot = torch.cuda.mem_get_info(dev)
+    tmp_bytes = int(4.5 * M * B * 8 * cw)
+    fit = int((free_b - nbytes - blk_bytes - tmp_bytes - (4 << 30)) // blk_bytes)
+    nres = max(2, min(nblk, fit)) if args.resident_blocks <= 0 else min(nblk, args.resident_blocks)
+    nres = min(nres, nblk)
 
     # inputs: seeded U[-0.5, 0.5] blocks, S-orthonormalised per block, Ritz values
     # from a per-block Rayleigh-Ritz, b_U from a 10-step Lanczos on H S^-1approx; all with the library's applies.
     gen = torch.Generator(device=dev).manual_seed(cfg.seed + 1000 * rank)
-    tdt = torch.float64 if prec == FP64 else torch.float32
-    # Large configs: keep at most `--resident-blocks` distinct blocks in HBM and cycle through them (the operators,
-    # the FP64 cell matrices of the residual set-up and the workspace leave no room for all N vectors of config 4;
-    # DESIGN.md section 7).  Every timed call still filters a block that is not in L2.
-    nres = nblk if args.resident_blocks <= 0 else min(nblk, args.resident_blocks)
     blocks, lams = [], []
     for b in range(nres):
         X0 = torch.rand(shape, dtype=torch.float64, device=dev, generator=gen) - 0.5
@@ -217,30 +240,29 @@ def run_own(args):
         blocks.append(X.to(tdt).contiguous())
         del X
         lams.append(lam)
+    torch.cuda.empty_cache()
     bU = hz.upper_bound(k=10, seed=1)
     b0 = min(l[0] for l in lams) - 0.1
     bW = min(max(l[-1] for l in lams), 0.5 * (b0 + bU))
-    blk_bytes = blocks[0].numel() * blocks[0].element_size()
-    nbytes = ctx.filter_workspace(prec, B)
     free_b, _tot = torch.cuda.mem_get_info(dev)
-    room = int((free_b - nbytes - (6 << 30)) // max(1, nres * blk_bytes))
+    room = int((free_b - nbytes - blk_bytes - (6 << 30)) // max(1, nres * blk_bytes))
     ring_n = max(1, min(args.steps + args.warmup, args.ring, room + 1))
     ring = [blocks] + [[x.clone() for x in blocks] for _ in range(ring_n - 1)]
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
-    # A block must not be filtered twice in place (the filter amplifies the wanted end of the spectrum by many orders
-    # of magnitude per call).  When blocks are reused (cycled resident blocks, or fewer ring copies than steps), each
-    # call filters a fresh device-to-device copy; the copy is inside the timed region (< 0.5% of a call).
+    # A block must not be filtered twice in place: with random (mid-spectrum) Ritz blocks the components below b0 grow by
+    # ~1e5 per call.  When blocks are reused (cycled resident blocks, or fewer ring copies than steps), each call filters a
+    # fresh device-to-device copy; the copy is inside the timed region (< 0.5% of a call).
     reuse = nres < nblk or ring_n < args.steps + args.warmup
     scratch = torch.empty_like(blocks[0]) if reuse else None
 
     def one_step(i):
         blks = ring[i % ring_n]
         for b in range(nblk):
-            x = blks[b % nres]
+            x, w = blks[b % nres], widths[b]
             if reuse:
                 scratch.copy_(x)
                 x = scratch
-            ctx.cheb_filter(prec, m, b0, bW, bU, x, lams[b % nres], B, B, ws, nbytes)
+            ctx.cheb_filter(prec, m, b0, bW, bU, x, lams[b % nres][:w], B, w, ws, nbytes)
 
     def barrier():
         if world > 1:
@@ -261,33 +283,59 @@ def run_own(args):
     barrier()
     ms = ev0.elapsed_time(ev1)
     ncell_launch, cell_ms = ctx.cell_timing_read()
+    nsetup, setup_ms = ctx.setup_timing_read()
     ctx.cell_timing(False)
     launches = ctx.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     ms = max_over_ranks(ms, world, dev)
     finite = all(bool(torch.isfinite(x).all()) for blks in ring for x in blks) and (scratch is None or bool(torch.isfinite(scratch).all()))
 
-    # end to end through the C ABI with HOST buffers: H2D of each block, filter, D2H of Psi_f, inside the timed region
+    # ---- end to end through the C ABI with HOST buffers: H2D of each block, filter, D2H of Psi_f, inside the timed region ----
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    # one pinned host copy of the block set per call (warm-up + e2e_steps): never filter a host block twice in place
-    host_sets = [[x.cpu().pin_memory() for x in ring[0]] for _ in range(1 + e2e_steps)]
+    cycled = nres < nblk
+    if cycled:
+        e2e_steps = 1
+    if not cycled:
+        # one pinned host copy of the block set per call (warm-up + e2e_steps): never filter a host block twice in place
+        host_sets = [[x.cpu().pin_memory() for x in ring[0]] for _ in range(1 + e2e_steps)]
+    else:
+        # cycled resident blocks: two pinned SOURCE blocks and two pinned WORK blocks; a helper thread refills the next work
+        # block from its source while the current one is filtered (in place) -- the host-side refill is not part of the path
+        src = [ring[0][k].cpu().pin_memory() for k in range(2)]
+        work = [torch.empty_like(src[0]).pin_memory() for _ in range(2)]
     del ring, blocks, ws, scratch  # the host-buffer call owns its own device block and workspace
     torch.cuda.empty_cache()
 
-    def one(k):
+    def e2e_pass_all(k):
         hs = host_sets[k]
-        if nres == nblk:
-            # the pass's blocks in one call: copies of blocks k+1 / k-1 run under block k's filter
-            ctx.cheb_filter_host_set(prec, m, b0, bW, bU, [x.data_ptr() for x in hs], lams, [B] * nblk, [B] * nblk)
-        else:   # cycled resident blocks (host blocks repeat): one block per call
-            for b in range(nblk):
-                ctx.cheb_filter_host(prec, m, b0, bW, bU, hs[b % nres].data_ptr(), lams[b % nres], B, B)
+        # the pass's blocks in one call: copies of blocks k+1 / k-1 run under block k's filter
+        ctx.cheb_filter_host_set(prec, m, b0, bW, bU, [x.data_ptr() for x in hs], [lams[b][:widths[b]] for b in range(nblk)],
+                                 [B] * nblk, widths)
 
-    one(0)
+    def e2e_pass_cycled(nb):
+        import threading
+        work[0].copy_(src[0])
+        for b in range(nb):
+            t = None
+            if b + 1 < nb:
+                t = threading.Thread(target=lambda q=(b + 1) % 2: work[q].copy_(src[q]))
+                t.start()
+            w = widths[b % nblk]
+            ctx.cheb_filter_host(prec, m, b0, bW, bU, work[b % 2].data_ptr(), lams[b % 2][:w], B, w)
+            if t is not None:
+                t.join()
+
+    if cycled:
+        e2e_pass_cycled(2)          # warm-up: sizes the library's internal device block and workspace
+    else:
+        e2e_pass_all(0)
     barrier()
     t0 = time.perf_counter()
     for k in range(e2e_steps):
-        one(1 + k)
+        if cycled:
+            e2e_pass_cycled(nblk)
+        else:
+            e2e_pass_all(1 + k)
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     e2e_s = max_over_ranks(e2e_s, world, dev)
@@ -301,44 +349,41 @@ def run_own(args):
     peaks = _peaks()
     n = (cfg.p + 1) ** 3
     ncell = cfg.ncells[0] * cfg.ncells[1] * cfg.ncells[2]
-    flops_launch = 2.0 * n * n * B * ncell * (4 if cplx else 1)
-    cell_avg_ms = cell_ms / max(1, ncell_launch)
     kname = ctx.cell_kernel_name(prec, B)
-    if "tcgen05" in kname:
-        peak = 0.5 * peaks["bf16_sust"]
-        peak_note = f"0.5 x {peaks['src']} sustained bf16 (TF32:bf16 nominal ratio)"
-        bound = "tensor"
+    fused = "tcgen05" in kname
+    passes = 3 if "3xtf32" in kname else 1
+    # the cell kernel is launched (m - 1) x passes times per filter call, each time on the call's own width
+    launches_per_step = sum(1 for _ in widths) * (m - 1) * passes
+    cell_avg_ms = cell_ms / max(1, ncell_launch)
+    Bavg = float(N) / nblk                         # mean block width of a pass (config 4: 19 x 256 + 136)
+    flops_launch = 2.0 * n * n * Bavg * ncell * (4 if cplx else 1)
+    tflops = flops_launch / (cell_avg_ms * 1e-3) / 1e12 if cell_avg_ms > 0 else 0.0
+    # Roofline of the dominant kernel.  k_cell_tcgen05 now IS the fused Chebyshev step (gather, S^-1approx
+    # through the K-extension, contraction, ordered assembly, bracket of Alg. 2 step 4), so its algorithmic bytes per launch
+    # are SURVEY.md 8(d)'s per-step figure: the H^e stream 4 n^2 N_c (x2 complex) + 20 B per dof*vec (read R_Y 4, R_X 4,
+    # Y FP64 8, write R_X 4; x2 complex).  FP32 mode (three passes): the same bytes per pass for the first pass.
+    bytes_launch = 4.0 * n * n * ncell * cw + 20.0 * M * Bavg * cw
+    gbs = bytes_launch / (cell_avg_ms * 1e-3) / 1e9 if cell_avg_ms > 0 else 0.0
+    if fused:
+        peak_t = 0.5 * peaks["bf16_sust"]
+        roof = {"kernel": f"k_cell_tcgen05 ({kname}: fused step)", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": gbs / peaks["hbm"], "traffic": None,
+                "traffic_source": "not measured in this run; ncu --set full captures per launch: profiles/r02_cell_kernel_ordered.md",
+                "peak_source": f"{peaks['src']} copy bandwidth", "algorithmic_bytes_per_launch": bytes_launch,
+                "algorithmic_bytes_per_dof_vec": bytes_launch / (M * Bavg),
+                "tensor": {"achieved_tflops": tflops, "peak_tflops": peak_t, "frac": tflops / peak_t,
+                           "peak_source": f"0.5 x {peaks['src']} sustained bf16 (nominal TF32:bf16 ratio; TF32 itself not measured)"}}
     else:
-        # SIMT FMA pipe: 148 SMs x 128 FP32 lanes x 2 flop at the clock seen under load
         mhz = (clocks or {}).get("sm_mhz") or 1965.0
         peak = 148 * 128 * 2 * mhz * 1e6 / 1e12 * (0.5 if prec == FP64 else 1.0)
-        peak_note = "148 SM x 128 lanes x 2 flop x SM clock under load (FP64: half, the DMMA / DFMA rate)"
-        bound = "tensor" if "dmma" in kname else "alu"
-    tflops = flops_launch / (cell_avg_ms * 1e-3) / 1e12 if cell_avg_ms > 0 else 0.0
-    # Roofline of the dominant kernel.  The fused tcgen05 step kernel is HBM-bound at these block
-    # widths: algorithmic bytes per launch = H^e stream (4 n^2 N_c, x2 complex) + read R_Y (4 B) +
-    # read-modify-write R_X (8 B) per dof*vec (x2 complex).  Other cell kernels: tensor / ALU flop rate.
-    cw = 2 if cplx else 1
-    bytes_launch = 4.0 * n * n * ncell * cw + 12.0 * M * B * cw
-    gbs = bytes_launch / (cell_avg_ms * 1e-3) / 1e9 if cell_avg_ms > 0 else 0.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "cell_kernel_traffic.csv")   # written from the committed ncu capture
-    if os.path.exists(tpath):
-        import csv
-        for row in csv.DictReader(open(tpath)):
-            if row["workload"] == cfg.name and row["kernel"] == kname and row["precision"] == args.prec:
-                traffic = float(row["dram_bytes_per_launch"])
-    if "tcgen05" in kname:
-        roof = {"kernel": kname, "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
-                "frac": gbs / peaks["hbm"], "traffic": traffic, "peak_source": f"{peaks['src']} copy bandwidth",
-                "algorithmic_bytes_per_launch": bytes_launch,
-                "tensor": {"achieved_tflops": tflops, "peak_tflops": peak, "frac": tflops / peak, "peak_source": peak_note}}
-    else:
-        roof = {"kernel": kname, "bound": bound, "achieved": tflops, "peak": peak, "unit": "TFLOP/s",
-                "frac": tflops / peak if peak else None, "traffic": traffic, "peak_source": peak_note}
+        roof = {"kernel": kname, "bound": "tensor" if "dmma" in kname else "alu", "achieved": tflops, "peak": peak, "unit": "TFLOP/s",
+                "frac": tflops / peak if peak else None, "traffic": None,
+                "peak_source": "148 SM x 128 lanes x 2 flop x SM clock under load (FP64: half, the DMMA / DFMA rate)"}
     roof.update({"launches": ncell_launch, "avg_ms": cell_avg_ms, "share_of_step": cell_ms / ms})
-    # whole-step HBM view: SURVEY.md 8(d) algorithmic bytes per dof*vec*step of the fully fused step
-    step_bytes = (4.0 * n * n * ncell * cw / (M * B) + 20.0 * cw)
+    # whole-step and recurrence-only views: total = a1-a8; recurrence-only = total minus the residual set-up
+    step_bytes = bytes_launch / (M * Bavg)
+    rec_ms = ms - setup_ms
+    rec_value = world * float(M) * N * (m - 1) * args.steps / (rec_ms * 1e-3) if rec_ms > 0 else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -346,18 +391,23 @@ def run_own(args):
         "config": {"workload": cfg.name, "dofs": M, "vectors": N, "block": B, "degree": m, "precision": args.prec,
                    "cells": ncell, "fe_order": cfg.p, "atoms": cfg.natoms, "projectors": cfg.nproj,
                    "pairs": ctx.num_pairs(), "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "cache": f"inputs >> L2: ring of {ring_n} copies of the {N}-vector block set "
-                            f"({ring_n * nres * blk_bytes / 2**30:.1f} GiB resident) + {nbytes / 2**30:.1f} GiB workspace per call",
+                   "cache": f"inputs >> L2: {nres} distinct resident blocks of {blk_bytes / 2**30:.2f} GiB x {ring_n} ring copies"
+                            f" + {nbytes / 2**30:.1f} GiB workspace; every timed call filters a block that is not in L2",
                    "resident_blocks": nres, "blocks_per_pass": nblk, "filters_fresh_copy": reuse,
                    "bounds": [b0, bW, bU], "finite": finite, "setup_s": t_setup},
         "clocks": clocks,
         "e2e": {"value": world * units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nblk * blk_bytes,
-                "d2h_bytes_per_step": nblk * blk_bytes, "steps": e2e_steps},
+                "d2h_bytes_per_step": nblk * blk_bytes, "steps": e2e_steps,
+                "how": "pawfe_cheb_filter_host per block (two pinned work blocks refilled by a helper thread)" if cycled
+                       else "pawfe_cheb_filter_host_set (copies pipelined under the filters)"},
         "gpu_launches": launches,
         "roofline": roof,
         "step_hbm": {"algorithmic_bytes_per_dof_vec_step": step_bytes,
                      "achieved_gbs": step_bytes * value / world / 1e9, "peak_gbs": peaks["hbm"],
                      "frac": step_bytes * value / world / 1e9 / peaks["hbm"]},
+        "phases": {"residual_setup_ms_per_step": setup_ms / args.steps, "residual_setup_share": setup_ms / ms,
+                   "recurrence_only_value": rec_value, "recurrence_only_unit": "dof*vec*(m-1 steps)/s, residual set-up excluded",
+                   "cell_kernel_launches_expected_per_step": launches_per_step, "filter_calls_timed": nsetup},
     }
     if world == 1 and not args.no_cpu_baseline:
         smp = OracleSample(args.config)
@@ -368,11 +418,21 @@ def run_own(args):
             smp.step()
             reps += 1
         dt = time.perf_counter() - t0
-        line["cpu_baseline"] = {"value": smp.units * reps / dt, "unit": UNIT, "cores": _cores_used(), "kind": "oracle",
-                                "sample": smp.desc + f"; {reps} calls in {dt:.1f} s"}
+        line["cpu_baseline"] = {"value": smp.units * reps / dt, "unit": UNIT, "cores": _cores_used(), "host_cores": _host_cores(),
+                                "kind": "oracle", "sample": smp.desc + f"; {reps} calls in {dt:.1f} s"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_all_configs(args):
+    """one line per config 1-4 (each in its own process, so that every config starts from an empty device)"""
+    for c in (1, 2, 3, 4):
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", str(args.steps), "--warmup", str(args.warmup),
+               "--prec", args.prec, "--no-cpu-baseline"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        out = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+        print(out[-1] if out else json.dumps({"config": c, "error": r.stderr[-500:]}), flush=True)
 
 
 def main():
@@ -381,15 +441,18 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--prec", default="tf32", choices=["fp64", "fp32", "tf32"])
     ap.add_argument("--ring", type=int, default=8)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--resident-blocks", type=int, default=0, help="distinct vector blocks kept in HBM (0 = all)")
     ap.add_argument("--block", type=int, default=0, help="override the config's block width B (0 = BASELINE.json's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true", help="one line per config 1-4, each in its own process")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.all_configs:
+        run_all_configs(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_own(args)

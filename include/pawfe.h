@@ -228,6 +228,10 @@ pawfe_status pawfe_launch_count(const pawfe_ctx* ctx, long* n);
  * and returns the number of launches recorded and the sum of their durations in milliseconds. */
 pawfe_status pawfe_cell_timing(pawfe_ctx* ctx, int enable);
 pawfe_status pawfe_cell_timing_read(pawfe_ctx* ctx, long* launches, double* ms);
+/* While pawfe_cell_timing is enabled every filter call also brackets its residual set-up (Alg. 2 steps 2-3, L260-L264: the
+ * FP64 products and the scaling into R_Y) with an event pair: number of filter calls recorded and the sum of their set-up
+ * times in milliseconds (bench.py's recurrence-only throughput = total minus this).  Synchronises the stream. */
+pawfe_status pawfe_setup_timing_read(pawfe_ctx* ctx, long* calls, double* ms);
 
 /* Name of the cell-contraction kernel variant a given (prec, B) runs ("tcgen05_tf32", "simt_fp32",
  * "dmma_fp64", ...).  Static string. */

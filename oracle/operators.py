@@ -127,11 +127,163 @@ def apply_H_rows(sysd, X, cells):
             dc = cen - sysd.pos[a]
             if cfg.bc == "periodic":
                 dc -= mesh.box * np.round(dc / mesh.box)
-            if np.linalg.norm(dc) > sysd.rc + np.sqrt(3.0) * float(np.max(mesh.h)):
+            # cheap reject, rigorous: a node of the sampled cell gets weight from any of the 27 cells around it, whose farthest
+            # point is 1.5 sqrt(3) h from the sampled cell's centre
+            if np.linalg.norm(dc) > sysd.rc + 1.5 * np.sqrt(3.0) * float(np.max(mesh.h)):
                 continue
             Ca, _ = paw.build_C(mesh, sysd, kpt, atoms=[a])
             Ca = Ca[:, a * npj:(a + 1) * npj]
             P = Ca.conj().T @ X
             acc += Ca[J0] @ (sysd.D[a] @ P)
+        out.append((J0, acc * mask[J0][:, None]))
+    return out
+
+
+def _box_cells_near_atom(mesh, cfg, pos_a, rc):
+    """Cells whose box comes within rc of the atom (minimum image when periodic): a cheap geometric SUPERSET of the cells
+    that hold projector weight; the exact set is decided by paw.atom_cell_block (None = no quadrature point inside rc)."""
+    per = cfg.bc == "periodic"
+    cand = []
+    for d in range(3):
+        lo = np.arange(mesh.ncells[d]) * mesh.h[d]
+        hi = lo + mesh.h[d]
+        best = np.full(mesh.ncells[d], np.inf)
+        for s in ((-1, 0, 1) if per else (0,)):
+            xs = pos_a[d] + s * mesh.box[d]
+            best = np.minimum(best, np.where(xs < lo, lo - xs, np.where(xs > hi, xs - hi, 0.0)))
+        cand.append([(c, best[c] ** 2) for c in range(mesh.ncells[d]) if best[c] < rc])
+    return [(cx, cy, cz) for cx, dx in cand[0] for cy, dy in cand[1] for cz, dz in cand[2] if dx + dy + dz < rc * rc]
+
+
+def _cell_neighbourhood(mesh, cfg, c):
+    out = set()
+    for dx in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dz in (-1, 0, 1):
+                q = [c[0] + dx, c[1] + dy, c[2] + dz]
+                if cfg.bc == "periodic":
+                    q = [q[i] % mesh.ncells[i] for i in range(3)]
+                elif any(q[i] < 0 or q[i] >= mesh.ncells[i] for i in range(3)):
+                    continue
+                out.add(tuple(q))
+    return out
+
+
+def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
+    """Sampled rows of  H S^-1approx X  (the operator Algorithm 2 iterates: Alg. 1 step 2; Eq. 28; Eq. 30,
+    L230) at full size, from the definitions, without forming any global matrix:
+
+        T      = M_D^-1 X - M_D^-1 sum_b C^b Delta^b_Sinv (C^b^dagger M_D^-1 X)                       (Eq. 28)
+        (H T)_J = sum_{e contains J} (H^e T_e)_{I(J)} + sum_a C^a_J (D^a (C^a^dagger T))              (Eq. 13, 16)
+
+    for the nodes J of each listed cell (cx, cy, cz).  T is evaluated only where it is needed: on the nodes of the 27 cells
+    around the sampled cell and on the supports of the atoms a that reach the sampled cell; the atoms b that enter T there are
+    all atoms whose projector cells touch (share a node with) those regions.  X needs only row indexing: X[J] for an integer
+    index array J must return the (len(J), B) rows as a NumPy array (a NumPy array does; tests pass a device-tensor wrapper).
+    op="H" returns the rows of H X instead (T = X on the free dofs): the same evaluation as apply_H_rows, for an X that can
+    only be indexed by rows.  Returns [(J0, rows)] like apply_H_rows."""
+    if op not in ("HSinv", "H"):
+        raise ValueError(op)
+    cfg = sysd.cfg
+    mesh = fe.Mesh(cfg.ncells, cfg.box, cfg.p, cfg.bc)
+    kpt = cfg.kpoint
+    ref = fe.reference_cell_matrices(mesh)
+    mask = mesh.interior_mask()
+    md_inv = np.where(mask, 1.0 / fe.lumped_mass(mesh), 0.0)
+    npj = len(sysd.proj_l)
+    natoms = len(sysd.pos)
+    dtype = complex if kpt is not None else float
+    box_cells = [set(_box_cells_near_atom(mesh, cfg, sysd.pos[a], sysd.rc)) for a in range(natoms)]
+    blocks = {}          # (atom, cell) -> C^{e,a dagger} block or None, evaluated on demand
+
+    def block(a, c):
+        if (a, c) not in blocks:
+            blocks[(a, c)] = paw.atom_cell_block(mesh, sysd, a, c[0], c[1], c[2], kpt)
+        return blocks[(a, c)]
+
+    def atom_pairs(a):
+        """[(cell nodes J, C^{e,a} = conj(block)^T with Dirichlet rows zeroed)] over the cells that hold weight of atom a"""
+        out = []
+        for c in sorted(box_cells[a]):
+            Cd = block(a, c)
+            if Cd is not None:
+                J = mesh.cell_nodes(*c)
+                out.append((J, np.conj(Cd).T * mask[J][:, None]))
+        return out
+
+    def project(a, rows_of):
+        """C^a^dagger V for a vector field given by rows_of(J) -> V[J]"""
+        P = np.zeros((npj, ncol), dtype=dtype)
+        for J, Ce in atom_pairs(a):
+            P += Ce.conj().T @ rows_of(J)
+        return P
+
+    out = []
+    for c0 in cells:
+        c0 = tuple(int(v) for v in c0)
+        J0 = mesh.cell_nodes(*c0)
+        ncol = np.asarray(X[J0[:1]]).shape[1]
+        near = _cell_neighbourhood(mesh, cfg, c0)
+        # atoms with weight on a node of the sampled cell: the assembled C^a_J sums over EVERY cell that contains J (Eq. 16-17),
+        # so an atom that only reaches a neighbour cell still contributes at the shared face / edge / corner nodes
+        A0 = [a for a in range(natoms) if box_cells[a] & near]
+        region = set(near)                                                     # cells on whose nodes T is needed
+        for a in A0:
+            region |= box_cells[a]
+        touch = set()
+        for c in region:
+            touch |= _cell_neighbourhood(mesh, cfg, c)                         # cells sharing a node with the region
+        Bset = [b for b in range(natoms) if box_cells[b] & touch] if op == "HSinv" else []
+        # W^b = Delta^b_Sinv C^b^dagger M_D^-1 X, with Delta^b_Sinv = (I + dS^b G^b)^-1 dS^b, G^b = C^b^dagger M_D^-1 C^b (Eq. 29, R10)
+        W = {}
+        for b in Bset:
+            prs = atom_pairs(b)
+            if not prs:
+                continue
+            # assemble the atom's sparse column block on its own nodes (a node shared by two of its cells gets both parts)
+            nodes = np.unique(np.concatenate([J for J, _ in prs]))
+            loc = {int(j): i for i, j in enumerate(nodes)}
+            Cb = np.zeros((len(nodes), npj), dtype=dtype)
+            for J, Ce in prs:
+                np.add.at(Cb, [loc[int(j)] for j in J], Ce)
+            G = Cb.conj().T @ (md_inv[nodes][:, None] * Cb)
+            dSinv = np.linalg.solve(np.eye(npj) + sysd.dS[b] @ G, sysd.dS[b].astype(dtype))
+            P1 = Cb.conj().T @ (md_inv[nodes][:, None] * np.asarray(X[nodes]))
+            W[b] = (nodes, Cb, dSinv @ P1)
+
+        def T_rows(J):
+            J = np.asarray(J)
+            if op == "H":
+                return mask[J][:, None] * np.asarray(X[J]).astype(dtype)
+            t = md_inv[J][:, None] * np.asarray(X[J]).astype(dtype)
+            pos = {int(j): i for i, j in enumerate(J)}
+            for b, (nodes, Cb, Wb) in W.items():
+                hit = [(pos[int(j)], i) for i, j in enumerate(nodes) if int(j) in pos]
+                if hit:
+                    ii = np.array([h[0] for h in hit])
+                    kk = np.array([h[1] for h in hit])
+                    t[ii] -= md_inv[J[ii]][:, None] * (Cb[kk] @ Wb)
+            return t
+
+        pos_in = {int(j): i for i, j in enumerate(J0)}
+        acc = np.zeros((mesh.n, ncol), dtype=dtype)
+        for c in sorted(near):
+            J = mesh.cell_nodes(*c)
+            hit = [(pos_in[int(j)], i) for i, j in enumerate(J) if int(j) in pos_in]
+            if not hit:
+                continue
+            He = fe.hamiltonian_cell_matrix(mesh, sysd, c[0], c[1], c[2], kpt, ref)
+            Ye = He @ (T_rows(J) * mask[J][:, None])
+            for (i0, i) in hit:
+                acc[i0] += Ye[i]
+        for a in A0:
+            prs = atom_pairs(a)
+            if not prs:
+                continue
+            P2 = project(a, T_rows)
+            for J, Ce in prs:
+                hit = [(pos_in[int(j)], i) for i, j in enumerate(J) if int(j) in pos_in]
+                for (i0, i) in hit:
+                    acc[i0] += Ce[i] @ (sysd.D[a] @ P2)
         out.append((J0, acc * mask[J0][:, None]))
     return out

@@ -28,7 +28,7 @@ SYMBOLS = [
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
-    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc",
+    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read",
 ]
 
 
@@ -83,6 +83,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_launch_count.argtypes = [vp, C.POINTER(C.c_long)]
     lib.pawfe_cell_timing.argtypes = [vp, C.c_int]
     lib.pawfe_cell_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
+    lib.pawfe_setup_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
     lib.pawfe_cell_kernel_name.argtypes = [vp, C.c_int, C.c_int]
     lib.pawfe_cell_kernel_name.restype = C.c_char_p
     for s in SYMBOLS:
@@ -210,6 +211,11 @@ class Context:
     def cell_timing_read(self):
         n, ms = C.c_long(), C.c_double()
         self._check(self.lib.pawfe_cell_timing_read(self._h, C.byref(n), C.byref(ms)), "pawfe_cell_timing_read")
+        return n.value, ms.value
+
+    def setup_timing_read(self):
+        n, ms = C.c_long(), C.c_double()
+        self._check(self.lib.pawfe_setup_timing_read(self._h, C.byref(n), C.byref(ms)), "pawfe_setup_timing_read")
         return n.value, ms.value
 
     def cell_kernel_name(self, prec: int, B: int) -> str:

@@ -376,6 +376,7 @@ extern "C" pawfe_status pawfe_cell_timing(pawfe_ctx* c, int enable) {
   if (!c) return PAWFE_EINVAL;
   c->prof_on = enable != 0;
   c->prof_used = 0;
+  c->prof_setup_used = 0;
   return PAWFE_OK;
 }
 
@@ -389,6 +390,20 @@ extern "C" pawfe_status pawfe_cell_timing_read(pawfe_ctx* c, long* launches, dou
     tot += t;
   }
   *launches = (long)(c->prof_used / 2);
+  *ms = tot;
+  return PAWFE_OK;
+}
+
+extern "C" pawfe_status pawfe_setup_timing_read(pawfe_ctx* c, long* calls, double* ms) {
+  if (!c || !calls || !ms) return PAWFE_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < c->prof_setup_used; i += 2) {
+    float t = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&t, c->prof_setup_ev[i], c->prof_setup_ev[i + 1]));
+    tot += t;
+  }
+  *calls = (long)(c->prof_setup_used / 2);
   *ms = tot;
   return PAWFE_OK;
 }

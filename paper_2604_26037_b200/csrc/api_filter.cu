@@ -121,6 +121,7 @@ pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double
 
   const int gs = 8 * c->sm_count;
   // ---- step 2: Y = H X - S X Lambda in FP64 (L260, L374) ----
+  prof_setup_mark(c, true);
   if (HXin && SXin) {   // the caller's products (pawfe_cheb_filter_hs): no operator application
     k_residual_from_products<<<gs, 256, 0, c->stream>>>(c->M, (long)W, W, cw, (const double*)HXin, (const double*)SXin, ld * cw, ds, (double*)Y64);
     KERNEL_CHECK(c, "k_residual_from_products");
@@ -133,6 +134,7 @@ pawfe_status filter_impl(pawfe_ctx* c, pawfe_prec prec, int m, double b0, double
   k_residual_init<RS><<<gs, 256, 0, c->stream>>>(c->M, W, cw, (double*)Y64, (const double*)nullptr, ds, z_over_e,
                                                  (RS*)RX, (RS*)RY);
   KERNEL_CHECK(c, "k_residual_init");
+  prof_setup_mark(c, false);
   // ---- step 4 ----
   for (int th = 2; th <= m; ++th) {
     TRY((pawfe_apply_Sinv_impl<TS, TS, TS>(c, RY, B, T, B, B)));

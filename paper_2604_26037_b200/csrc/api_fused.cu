@@ -29,6 +29,7 @@ struct FusedPlan {
   // scratch for block width <= Bcap
   int Bcap = 0; long ldw = 0;
   float* d_P1 = nullptr;        // [natoms][npj][ldw]
+  float* d_Ppart = nullptr;     // [npairs][npj][ldw] per-pair partial projections (summed in pair order by k_psum)
   float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
   float* d_Wcat_lo = nullptr;   // low parts of Wcat (FP32 mode, 3xTF32 split)
   float* d_Bext_lo = nullptr;   // low parts of d_Bext (built on first FP32-mode use)
@@ -189,7 +190,7 @@ template <int NPJ>
 __global__ void __launch_bounds__(256, (NPJ <= 9 ? 3 : 2))
 k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
         const float* __restrict__ Cd, const float* __restrict__ X, long ldx, int B,
-        float* __restrict__ P, long ldp) {
+        float* __restrict__ P, long ldp, float* __restrict__ Ppart) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int n = md.n, n1 = md.n1;
   long* nodeO = reinterpret_cast<long*>(smem_raw);     // byte offset of the node's row, -1: masked
@@ -251,10 +252,39 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
     const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
     if (vv < B) {
       const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
-      float* dst = P + ((long)a * NPJ + al) * ldp + vv;
-      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
+      if (Ppart) {   // this pair's partial projection; k_psum adds the atom's pairs in a fixed order (bit-reproducible)
+        *reinterpret_cast<float4*>(Ppart + ((long)pr * NPJ + al) * ldp + vv) = val;
+      } else {
+        float* dst = P + ((long)a * NPJ + al) * ldp + vv;
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
+      }
     }
   }
+}
+
+// P[a][al][.] = sum over the atom's pairs, in pair order, of the per-pair partial projections (k_proj2 / k_projF with Ppart):
+// the ordered replacement of their cross-CTA reductions.  grid = (natoms * npj, ceil(Wq / 128)), block = 128; Wq = quads
+// of 4 real columns that hold data; ldq = leading dimension / 4.
+__global__ void __launch_bounds__(128)
+k_psum(int npj, const int* __restrict__ aps, const float4* __restrict__ Ppart, long ldq, int Wq, float4* __restrict__ P) {
+  const int a = blockIdx.x / npj, al = blockIdx.x - a * npj;
+  const int q = blockIdx.y * 128 + threadIdx.x;
+  if (q >= Wq) return;
+  float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+  const int p0 = aps[a], p1 = aps[a + 1];
+  int pr = p0;
+  for (; pr + 4 <= p1; pr += 4) {   // four loads in flight, added in pair order
+    float4 t[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) t[u] = Ppart[((long)(pr + u) * npj + al) * ldq + q];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { s.x += t[u].x; s.y += t[u].y; s.z += t[u].z; s.w += t[u].w; }
+  }
+  for (; pr < p1; ++pr) {
+    const float4 t = Ppart[((long)pr * npj + al) * ldq + q];
+    s.x += t.x; s.y += t.y; s.z += t.z; s.w += t.w;
+  }
+  P[((long)a * npj + al) * ldq + q] = s;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -312,94 +342,89 @@ k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, int Bpad,
   if (wr) Wa[(long)(npj + al) * ldw + v] = w2;
 }
 
-// X[J][v] += scale * M_D^-1[J] * sum_al C^{e,a}[I][al] W^a[al][v] over the pairs (recovery: scale = -1).
-//   grid = (npairs, ceil(B/128)), block = 256.  dynamic smem: n longs + n floats + npj*n floats.
+
+// Alg. 2 step 5 (L282) in one ORDERED pass:  X <- keep * (Rt_Y + X Lambda_Y) - M_D^-1 C W   (W = rows [0, npj) of Wcat).
+// Every node has one owner cell (local index < p in each direction; the upper wall planes of a Dirichlet mesh go to the last
+// cells); the owner's CTA sums, for each of its nodes, the low-rank contributions of ALL (cell, atom) pairs whose cell
+// contains the node -- the owner cell and the up to 7 cells below it -- in a fixed order (octant, then pair), and stores
+// the row once.  No atomics: the result is bit-reproducible, and the diagonal part needs no kernel of its own.
+//   grid = (ncell, ceil(Wr / 128)), block = 256: warp = node, lane = 4 consecutive real columns.  VEC: 16-byte accesses
+//   (ldx % 4 == 0, X 16-byte aligned); otherwise scalar accesses with a guard on the block's last quad.
+template <bool CPLX, bool VEC>
 __global__ void __launch_bounds__(256)
-k_scatter2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
-           const float* __restrict__ Cd, int npj, const float* __restrict__ Wcat, long ldw, int B, float scale,
-           float* __restrict__ X, long ldx) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int n = md.n, n1 = md.n1;
-  long* nodeJ = reinterpret_cast<long*>(smem_raw);
-  float* nodeS = reinterpret_cast<float*>(nodeJ + n);
-  float* Cs = nodeS + n;
-  const int pr = blockIdx.x, a = pair_atom[pr];
-  int cx, cy, cz;
-  mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
-  for (int I = threadIdx.x; I < n; I += blockDim.x) {
-    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
-    nodeJ[I] = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-    nodeS[I] = scale * (float)(md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz]);
-  }
-  for (int i = threadIdx.x; i < npj * n; i += blockDim.x) Cs[i] = Cd[(long)pr * npj * n + i];
-  __syncthreads();
+k_recover_ordered(MeshDev md, const int* __restrict__ cps, const int* __restrict__ cpi, const int* __restrict__ pair_atom,
+                  const float* __restrict__ Cd, int npj, const float* __restrict__ Wcat, long ldwc, const float* __restrict__ RY,
+                  long ldw, float* __restrict__ X, long ldx, int Wr, const double* __restrict__ lamY) {
+  constexpr int cw = CPLX ? 2 : 1;
+  const int n = md.n, n1 = md.n1, p = md.p;
+  const int e = blockIdx.x;
+  int cc[3];
+  mesh_cell_coords(md, e, &cc[0], &cc[1], &cc[2]);
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int v = blockIdx.y * 128 + lane * 4;
-  if (v >= B) return;
-  const bool vec = (ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0;   // rows 16-byte aligned
-  float4 wv[PAWFE_MAX_NPJ];
+  if (v >= Wr) return;
+  double lam[4];
 #pragma unroll
-  for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
-    wv[al] = al < npj ? *reinterpret_cast<const float4*>(Wcat + ((long)a * 32 + al) * ldw + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int u = 0; u < 4; ++u) lam[u] = v + u < Wr ? lamY[(v + u) / cw] : 0.0;
+  const bool last[3] = {!md.periodic && cc[0] == md.nc[0] - 1, !md.periodic && cc[1] == md.nc[1] - 1, !md.periodic && cc[2] == md.nc[2] - 1};
   for (int I = w; I < n; I += 8) {
-    const float s = nodeS[I];
-    if (s == 0.f) continue;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-    for (int al = 0; al < PAWFE_MAX_NPJ; ++al)
-      if (al < npj) {
-        const float cv = Cs[al * n + I];
-        acc.x = fmaf(cv, wv[al].x, acc.x); acc.y = fmaf(cv, wv[al].y, acc.y);
-        acc.z = fmaf(cv, wv[al].z, acc.z); acc.w = fmaf(cv, wv[al].w, acc.w);
-      }
-    float* dst = X + nodeJ[I] * ldx + v;
-    if (vec && v + 3 < B) {   // one 16-byte reduction instead of four scalar ones
-      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(s * acc.x), "f"(s * acc.y), "f"(s * acc.z), "f"(s * acc.w) : "memory");
-    } else {
-      atomicAdd(dst + 0, s * acc.x);
-      if (v + 1 < B) atomicAdd(dst + 1, s * acc.y);
-      if (v + 2 < B) atomicAdd(dst + 2, s * acc.z);
-      if (v + 3 < B) atomicAdd(dst + 3, s * acc.w);
-    }
-  }
-}
-
-__device__ inline double mdinv_row(const MeshDev& md, long J) {
-  int iz = (int)(J % md.N[2]);
-  long t = J / md.N[2];
-  int iy = (int)(t % md.N[1]);
-  int ix = (int)(t / md.N[1]);
-  return md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
-}
-
-// Alg. 2 step 5 (L282), diagonal part:  X <- keep * (Rt_Y + X Lambda_Y);  the low-rank part of S^-1approx R_Y is added
-// by k_scatter2.  keep = 0 on Dirichlet boundary rows.  VEC: 4 consecutive columns per thread (needs ldx % 4 == 0 and a
-// 16-byte aligned X; the columns beyond B of a ragged last quad are the caller's and are left untouched).
-template <bool VEC>
-__global__ void __launch_bounds__(256)
-k_recover2(MeshDev md, long ldw, int B /*real columns*/, int cw, const float* __restrict__ RY, float* __restrict__ X,
-           long ldx, const double* __restrict__ lamY) {
-  const int nq = (B + 3) / 4;
-  const long total = md.M * (long)nq;
-  for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
-    const long J = idx / nq;
-    const int v = (int)(idx - J * nq) * 4;
-    const double keep = mdinv_row(md, J) != 0.0 ? 1.0 : 0.0;
-    const float4 ry = *reinterpret_cast<const float4*>(RY + J * ldw + v);   // ldw % 4 == 0, pad columns readable
+    const int loc[3] = {I / (n1 * n1), (I / n1) % n1, I % n1};
+    if ((loc[0] == p && !last[0]) || (loc[1] == p && !last[1]) || (loc[2] == p && !last[2])) continue;   // another cell owns it
+    int ix, iy, iz;
+    const long J = mesh_node(md, cc[0], cc[1], cc[2], loc[0], loc[1], loc[2], &ix, &iy, &iz);
+    const double mi = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz];
     float* xp = X + J * ldx + v;
-    if (VEC && v + 3 < B) {
-      const float4 x = *reinterpret_cast<const float4*>(xp);
-      float4 o;
-      o.x = (float)(keep * ((double)ry.x + (double)x.x * lamY[v / cw]));
-      o.y = (float)(keep * ((double)ry.y + (double)x.y * lamY[(v + 1) / cw]));
-      o.z = (float)(keep * ((double)ry.z + (double)x.z * lamY[(v + 2) / cw]));
-      o.w = (float)(keep * ((double)ry.w + (double)x.w * lamY[(v + 3) / cw]));
-      *reinterpret_cast<float4*>(xp) = o;
-    } else {
-      const float r[4] = {ry.x, ry.y, ry.z, ry.w};
+    float xo[4] = {0.f, 0.f, 0.f, 0.f};
+    if (mi != 0.0) {   // (Dirichlet wall rows are written as 0)
+      const float4 ry = *reinterpret_cast<const float4*>(RY + J * ldw + v);   // ldw % 4 == 0, pad columns readable
+      float xi[4];
+      if (VEC) { const float4 t = *reinterpret_cast<const float4*>(xp); xi[0] = t.x; xi[1] = t.y; xi[2] = t.z; xi[3] = t.w; }
+      else {
 #pragma unroll
-      for (int u = 0; u < 4; ++u)
-        if (v + u < B) xp[u] = (float)(keep * ((double)r[u] + (double)xp[u] * lamY[(v + u) / cw]));
+        for (int u = 0; u < 4; ++u) xi[u] = v + u < Wr ? xp[u] : 0.f;
+      }
+      xo[0] = (float)((double)ry.x + (double)xi[0] * lam[0]); xo[1] = (float)((double)ry.y + (double)xi[1] * lam[1]);
+      xo[2] = (float)((double)ry.z + (double)xi[2] * lam[2]); xo[3] = (float)((double)ry.w + (double)xi[3] * lam[3]);
+      const float s = -(float)mi;
+      for (int oct = 0; oct < 8; ++oct) {
+        const int d[3] = {oct & 1, (oct >> 1) & 1, (oct >> 2) & 1};
+        if ((d[0] && loc[0] != 0) || (d[1] && loc[1] != 0) || (d[2] && loc[2] != 0)) continue;   // the node is not on that face
+        int c2[3], l2[3];
+        bool ok = true;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          c2[k] = cc[k] - d[k];
+          l2[k] = d[k] ? p : loc[k];
+          if (c2[k] < 0) { if (md.periodic) c2[k] += md.nc[k]; else ok = false; }
+        }
+        if (!ok) continue;
+        const int e2 = (c2[0] * md.nc[1] + c2[1]) * md.nc[2] + c2[2];
+        const int I2 = (l2[0] * n1 + l2[1]) * n1 + l2[2];
+        for (int q = cps[e2]; q < cps[e2 + 1]; ++q) {
+          const int pr = cpi[q], at = pair_atom[pr];
+          float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+          for (int al = 0; al < npj; ++al) {
+            const float4 wv = *reinterpret_cast<const float4*>(Wcat + ((long)at * 32 + al) * ldwc + v);
+            if (CPLX) {   // conj(Cd) * W on interleaved (re, im) columns
+              const float2 cv = *reinterpret_cast<const float2*>(Cd + (((long)pr * npj + al) * n + I2) * 2);
+              acc.x = fmaf(cv.x, wv.x, acc.x); acc.x = fmaf(cv.y, wv.y, acc.x);
+              acc.y = fmaf(cv.x, wv.y, acc.y); acc.y = fmaf(-cv.y, wv.x, acc.y);
+              acc.z = fmaf(cv.x, wv.z, acc.z); acc.z = fmaf(cv.y, wv.w, acc.z);
+              acc.w = fmaf(cv.x, wv.w, acc.w); acc.w = fmaf(-cv.y, wv.z, acc.w);
+            } else {
+              const float cv = Cd[((long)pr * npj + al) * n + I2];
+              acc.x = fmaf(cv, wv.x, acc.x); acc.y = fmaf(cv, wv.y, acc.y);
+              acc.z = fmaf(cv, wv.z, acc.z); acc.w = fmaf(cv, wv.w, acc.w);
+            }
+          }
+          xo[0] += s * acc.x; xo[1] += s * acc.y; xo[2] += s * acc.z; xo[3] += s * acc.w;
+        }
+      }
+    }
+    if (VEC) *reinterpret_cast<float4*>(xp) = make_float4(xo[0], xo[1], xo[2], xo[3]);
+    else {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (v + u < Wr) xp[u] = xo[u];
     }
   }
 }
@@ -408,7 +433,7 @@ void free_plan(FusedPlan* p) {
   if (!p) return;
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
   cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD); cudaFree(p->d_cps); cudaFree(p->d_cpi);
-  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
+  cudaFree(p->d_P1); cudaFree(p->d_Ppart); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
   cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
   if (p->aux) cudaStreamDestroy(p->aux);
   if (p->ev_fork) cudaEventDestroy(p->ev_fork);
@@ -466,10 +491,13 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   for (int a = 0; a < natoms; ++a) { for (int b : nbs[a]) na.push_back(b); ns[a + 1] = (int)na.size(); }
   const long nnb = (long)na.size();
   p->ext_ksteps = (2 * npj + 7) / 8;
-  if (p->nchunks == 0) { p->ok = true; return PAWFE_OK; }
+  if (p->nchunks == 0) {   // no atoms near any cell: only the cell -> pairs lists (all empty) are needed, by the recovery kernel
+    TRY(upload(c, &p->d_cps, cps)); TRY(upload(c, &p->d_cpi, cpi));
+    p->ok = true; return PAWFE_OK;
+  }
 
   int* d_ec = nullptr;
-  int *&d_cps = p->d_cps, *&d_cpi = p->d_cpi;   // kept: the fused prepass + projection kernel walks the cells' pairs
+  int *&d_cps = p->d_cps, *&d_cpi = p->d_cpi;   // kept: the ordered recovery kernel walks the cells' pairs
   double* d_G = nullptr;
   pawfe_status st = PAWFE_OK;
   auto cleanup = [&]() { cudaFree(d_ec); cudaFree(d_G); };
@@ -545,12 +573,13 @@ pawfe_status ensure_scratch(pawfe_ctx* c, FusedPlan* p, int Bvec) {
   if (B <= p->Bcap) return PAWFE_OK;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   if (p->aux) CUDA_TRY(c, cudaStreamSynchronize(p->aux));
-  cudaFree(p->d_P1); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64); cudaFree(p->d_Wcat_lo);
-  p->d_Wcat_lo = nullptr;
+  cudaFree(p->d_P1); cudaFree(p->d_Ppart); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64); cudaFree(p->d_Wcat_lo);
+  p->d_Wcat_lo = nullptr; p->d_Ppart = nullptr;
   p->d_P1 = p->d_Wcat = nullptr; p->d_P64 = p->d_W64 = nullptr; p->Bcap = 0;
   const long ldw = roundup4(B);
   const size_t na = (size_t)std::max(1, c->natoms);
   TRY(dev_alloc(c, &p->d_P1, na * c->npj * ldw));
+  TRY(dev_alloc(c, &p->d_Ppart, (size_t)std::max<long>(1, c->npairs) * c->npj * ldw));
   TRY(dev_alloc(c, &p->d_Wcat, na * 32 * ldw));
   TRY(dev_alloc(c, &p->d_Wcat_lo, na * 32 * ldw));
   TRY(dev_alloc(c, &p->d_P64, na * c->npj * ldw));
@@ -577,7 +606,7 @@ pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, 
   const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)NPJ * n * 2 + 3) / 4 * 16 + (size_t)NPJ * 128 * 4;
   TRY(pawfe_ensure_smem(c, (const void*)k_projF<NPJ, true>, smem));
   k_projF<NPJ, true><<<dim3((unsigned)c->npairs, ceil_div(Wr, 128)), 256, smem, c->stream>>>(
-      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw);
+      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw, p->d_Ppart);
   KERNEL_CHECK(c, "k_projF");
   return PAWFE_OK;
 }
@@ -586,7 +615,14 @@ pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, 
 pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
-  CUDA_TRY(c, cudaMemsetAsync(p->d_P1, 0, (size_t)c->natoms * npj * p->ldw * sizeof(float), c->stream));
+  // per-pair partial projections, then their sum in pair order (no cross-CTA reductions: bit-reproducible)
+  auto psum = [&](int Wr) -> pawfe_status {
+    const int Wq = (Wr + 3) / 4;
+    k_psum<<<dim3((unsigned)(c->natoms * npj), ceil_div(Wq, 128)), 128, 0, c->stream>>>(
+        npj, c->d_atom_pair_start, (const float4*)p->d_Ppart, p->ldw / 4, Wq, (float4*)p->d_P1);
+    KERNEL_CHECK(c, "k_psum");
+    return PAWFE_OK;
+  };
   if (c->cplx) {
     switch (npj) {
 #define CASE_PC(N) case N: TRY(project_cplx<N>(c, p, X, ldx, 2 * B)); break;
@@ -594,6 +630,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
       CASE_PC(9) CASE_PC(10) CASE_PC(11) CASE_PC(12) CASE_PC(13) CASE_PC(14) CASE_PC(15) CASE_PC(16)
 #undef CASE_PC
     }
+    TRY(psum(2 * B));
     const int Bpad = (int)(roundup4(2 * B) / 2);
     k_couple<float2><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
         npj, mode, (const float2*)p->d_P1, p->ldw / 2, B, Bpad, (const float2*)c->d_dSinv32, (const float2*)c->d_D32, p->d_nb_start,
@@ -606,7 +643,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
 #define LAUNCH_PROJ2(NPJ)                                                                                            \
   do {                                                                                                               \
     TRY(pawfe_ensure_smem(c, (const void*)k_proj2<NPJ>, smem)); \
-    k_proj2<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw); \
+    k_proj2<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw, p->d_Ppart); \
   } while (0)
   switch (npj) {
     case 1: LAUNCH_PROJ2(1); break;   case 2: LAUNCH_PROJ2(2); break;   case 3: LAUNCH_PROJ2(3); break;
@@ -618,6 +655,7 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   }
 #undef LAUNCH_PROJ2
   KERNEL_CHECK(c, "k_proj2");
+  TRY(psum(B));
   const int Bpad = (int)roundup4(B);
   k_couple<float><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
       npj, mode, p->d_P1, p->ldw, B, Bpad, (const float*)c->d_dSinv32, (const float*)c->d_D32, p->d_nb_start, p->d_nb_atom,
@@ -799,18 +837,6 @@ pawfe_status fused_apply_HSinv(pawfe_ctx* c, pawfe_prec prec, const float* X, lo
   return cell_pass(c, p, prec, p->d_xs, lds, Y, ldy, Wr, 1.0f, 0, epi_plain(TC_EPI_STORE), p->d_xlo);
 }
 
-// recovery's low-rank part for complex contexts:  X -= M_D^-1 C W  (W = rows [0, npj) of Wcat)
-template <int NPJ>
-static pawfe_status scatter_cplx(pawfe_ctx* c, FusedPlan* p, float* X, long ldx, int Wr) {
-  const int n = c->n;
-  const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)NPJ * n * 2 + 3) / 4 * 16;
-  TRY(pawfe_ensure_smem(c, (const void*)k_scatterF<NPJ, true>, smem));
-  k_scatterF<NPJ, true><<<dim3((unsigned)c->npairs, ceil_div(Wr, 128)), 256, smem, c->stream>>>(
-      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, p->d_Wcat, p->ldw, 32, Wr, 1, -1.0f, X, ldx);
-  KERNEL_CHECK(c, "k_scatterF");
-  return PAWFE_OK;
-}
-
 // Step 2 of Alg. 2 for real contexts (L260, L374), FP64, S X never stored:  Yt <- H X - S X Lambda  (unscaled; the caller
 // scales).  The DMMA product runs on the context's stream, the mass sweeps and the FP64 non-local part (both add into Yt
 // with FP64 atomics) on the auxiliary stream; on any failure the auxiliary stream is joined before returning.
@@ -863,6 +889,7 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   const double* lam = ds;
   const double* neg_lam = ds + (size_t)(m + 1) * B;
   // ---- step 2 (FP64, L260, L374): Y = H X - S X Lambda ----
+  prof_setup_mark(c, true);
   if (HX && SX) {
     k_residual_from_products<<<gs, 256, 0, c->stream>>>(c->M, ldw, Wr, cw, (const double*)HX, (const double*)SX, ldx, lam, Yt);
     KERNEL_CHECK(c, "k_residual_from_products");
@@ -876,6 +903,7 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   // ---- step 3 in the scaled variables: Yt = M_D^-1 Y, Rt_Y = (zeta/e) Yt, Rt_X = 0 (pad columns 0) ----
   k_residual_init3<<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, Yt, z_over_e, RX, RY);
   KERNEL_CHECK(c, "k_residual_init3");
+  prof_setup_mark(c, false);
   // ---- step 4: one projection + coupling pass and ONE cell kernel per step; the cell kernel's first writers store the
   //      bracket  -a c Rt_Y - zeta zeta1 Rt_X [FP32] + Yt (a Lambda_Y) [FP64 add, L374]  plus their own share of
   //      a M_D^-1 H T, the other cells add theirs in cell order ----
@@ -888,24 +916,16 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----
   TRY(project_and_couple(c, p, RY, ldw, B, 1));
-  if ((ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0)
-    k_recover2<true><<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
-  else
-    k_recover2<false><<<gs, 256, 0, c->stream>>>(c->md, ldw, Wr, cw, RY, X, ldx, ds + (size_t)m * B);
-  KERNEL_CHECK(c, "k_recover2");
-  if (c->npairs > 0 && c->cplx) {
-    switch (c->npj) {
-#define CASE_SC(N) case N: TRY(scatter_cplx<N>(c, p, X, ldx, Wr)); break;
-      CASE_SC(1) CASE_SC(2) CASE_SC(3) CASE_SC(4) CASE_SC(5) CASE_SC(6) CASE_SC(7) CASE_SC(8)
-      CASE_SC(9) CASE_SC(10) CASE_SC(11) CASE_SC(12) CASE_SC(13) CASE_SC(14) CASE_SC(15) CASE_SC(16)
-#undef CASE_SC
-    }
-  } else if (c->npairs > 0) {
-    size_t smem = (size_t)c->n * 12 + (size_t)c->npj * c->n * 4;
-    TRY(pawfe_ensure_smem(c, (const void*)k_scatter2, smem));
-    k_scatter2<<<dim3((unsigned)c->npairs, ceil_div(B, 128)), 256, smem, c->stream>>>(
-        c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, c->npj, p->d_Wcat, p->ldw, B, -1.0f, X, ld);
-    KERNEL_CHECK(c, "k_scatter2");
+  {
+    const bool vec = (ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0;
+    const dim3 grid((unsigned)c->ncell, ceil_div(Wr, 128));
+    const double* lamY = ds + (size_t)m * B;
+#define LAUNCH_REC(CP, VE) k_recover_ordered<CP, VE><<<grid, 256, 0, c->stream>>>(c->md, p->d_cps, p->d_cpi, c->d_pair_atom, \
+        (const float*)c->d_Cd32, c->npj, p->d_Wcat, p->ldw, RY, ldw, X, ldx, Wr, lamY)
+    if (c->cplx) { if (vec) LAUNCH_REC(true, true); else LAUNCH_REC(true, false); }
+    else { if (vec) LAUNCH_REC(false, true); else LAUNCH_REC(false, false); }
+#undef LAUNCH_REC
+    KERNEL_CHECK(c, "k_recover_ordered");
   }
   return PAWFE_OK;
 }

@@ -187,6 +187,8 @@ struct pawfe_ctx {
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;  // pairs (start, stop)
   size_t prof_used = 0;
+  std::vector<cudaEvent_t> prof_setup_ev;  // pairs around the residual set-up (Alg. 2 steps 2-3) of every filter call
+  size_t prof_setup_used = 0;
 
   void* d_tmpblk = nullptr; size_t tmpblk_bytes = 0;   // block T of the unfused pawfe_apply_HSinv
 

@@ -49,3 +49,15 @@ static inline void prof_end(pawfe_ctx* c) {
   cudaEventRecord(c->prof_ev[c->prof_used + 1], c->stream);
   c->prof_used += 2;
 }
+
+// the same around the residual set-up of a filter call (Alg. 2 steps 2-3): bench.py's recurrence-only figure
+static inline void prof_setup_mark(pawfe_ctx* c, bool begin) {
+  if (!c->prof_on) return;
+  if (begin && c->prof_setup_used + 2 > c->prof_setup_ev.size()) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    c->prof_setup_ev.push_back(a); c->prof_setup_ev.push_back(b);
+  }
+  if (begin) cudaEventRecord(c->prof_setup_ev[c->prof_setup_used], c->stream);
+  else { cudaEventRecord(c->prof_setup_ev[c->prof_setup_used + 1], c->stream); c->prof_setup_used += 2; }
+}

@@ -102,6 +102,7 @@ extern "C" pawfe_status pawfe_destroy(pawfe_ctx* c) {
   }
   if (c->h_stage) cudaFreeHost(c->h_stage);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
+  for (cudaEvent_t e : c->prof_setup_ev) cudaEventDestroy(e);
   delete c;
   return PAWFE_OK;
 }
