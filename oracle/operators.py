@@ -169,7 +169,36 @@ def _cell_neighbourhood(mesh, cfg, c):
     return out
 
 
-def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
+def atom_pair_blocks(sysd, a):
+    """[(cell (cx, cy, cz), C^{e,a dagger} block)] over the cells that hold weight of atom a (paw.atom_cell_block, Eq. 34).
+    Module-level and free of shared state so that a test can evaluate many atoms in parallel worker processes."""
+    cfg = sysd.cfg
+    mesh = fe.Mesh(cfg.ncells, cfg.box, cfg.p, cfg.bc)
+    out = []
+    for c in sorted(_box_cells_near_atom(mesh, cfg, sysd.pos[a], sysd.rc)):
+        Cd = paw.atom_cell_block(mesh, sysd, a, c[0], c[1], c[2], cfg.kpoint)
+        if Cd is not None:
+            out.append((c, Cd))
+    return out
+
+
+def atoms_near_cells(sysd, cells, radius):
+    """atoms whose (minimum-image) distance to the centre of one of the cells is below radius"""
+    cfg = sysd.cfg
+    mesh = fe.Mesh(cfg.ncells, cfg.box, cfg.p, cfg.bc)
+    out = []
+    for a in range(len(sysd.pos)):
+        for c in cells:
+            d = mesh.cell_origin(*c) + 0.5 * mesh.h - sysd.pos[a]
+            if cfg.bc == "periodic":
+                d -= mesh.box * np.round(d / mesh.box)
+            if np.linalg.norm(d) < radius:
+                out.append(a)
+                break
+    return out
+
+
+def apply_HSinv_rows(sysd, X, cells, op="HSinv", cache=None):
     """Sampled rows of  H S^-1approx X  (the operator Algorithm 2 iterates: Alg. 1 step 2; Eq. 28; Eq. 30,
     L230) at full size, from the definitions, without forming any global matrix:
 
@@ -181,7 +210,9 @@ def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
     all atoms whose projector cells touch (share a node with) those regions.  X needs only row indexing: X[J] for an integer
     index array J must return the (len(J), B) rows as a NumPy array (a NumPy array does; tests pass a device-tensor wrapper).
     op="H" returns the rows of H X instead (T = X on the free dofs): the same evaluation as apply_H_rows, for an X that can
-    only be indexed by rows.  Returns [(J0, rows)] like apply_H_rows."""
+    only be indexed by rows.  cache: an optional dict that keeps the projector blocks and cell matrices between calls on the
+    same system (they do not depend on X or op); cache["blocks"][a] may be pre-filled with atom_pair_blocks(sysd, a).
+    Returns [(J0, rows)] like apply_H_rows."""
     if op not in ("HSinv", "H"):
         raise ValueError(op)
     cfg = sysd.cfg
@@ -194,22 +225,29 @@ def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
     natoms = len(sysd.pos)
     dtype = complex if kpt is not None else float
     box_cells = [set(_box_cells_near_atom(mesh, cfg, sysd.pos[a], sysd.rc)) for a in range(natoms)]
-    blocks = {}          # (atom, cell) -> C^{e,a dagger} block or None, evaluated on demand
-
-    def block(a, c):
-        if (a, c) not in blocks:
-            blocks[(a, c)] = paw.atom_cell_block(mesh, sysd, a, c[0], c[1], c[2], kpt)
-        return blocks[(a, c)]
+    cache = {} if cache is None else cache
+    pairs_of = cache.setdefault("atom_pairs", {})      # atom -> [(J, C^{e,a})], evaluated on demand
+    He_of = cache.setdefault("He", {})                 # cell -> H^e
 
     def atom_pairs(a):
         """[(cell nodes J, C^{e,a} = conj(block)^T with Dirichlet rows zeroed)] over the cells that hold weight of atom a"""
-        out = []
-        for c in sorted(box_cells[a]):
-            Cd = block(a, c)
-            if Cd is not None:
+        if a not in pairs_of:
+            raw = cache.get("blocks", {}).get(a)
+            if raw is None:
+                raw = atom_pair_blocks(sysd, a)
+            out = []
+            for c, Cd in raw:
                 J = mesh.cell_nodes(*c)
                 out.append((J, np.conj(Cd).T * mask[J][:, None]))
-        return out
+            pairs_of[a] = out
+        return pairs_of[a]
+
+    def rows_in(J, nodes):
+        """positions (in J, in the sorted array nodes) of the entries of J that occur in nodes"""
+        k = np.searchsorted(nodes, J)
+        k[k == len(nodes)] = 0
+        ii = np.nonzero(nodes[k] == J)[0]
+        return ii, k[ii]
 
     def project(a, rows_of):
         """C^a^dagger V for a vector field given by rows_of(J) -> V[J]"""
@@ -241,11 +279,10 @@ def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
             if not prs:
                 continue
             # assemble the atom's sparse column block on its own nodes (a node shared by two of its cells gets both parts)
-            nodes = np.unique(np.concatenate([J for J, _ in prs]))
-            loc = {int(j): i for i, j in enumerate(nodes)}
+            nodes = np.unique(np.concatenate([J for J, _ in prs]))          # sorted
             Cb = np.zeros((len(nodes), npj), dtype=dtype)
             for J, Ce in prs:
-                np.add.at(Cb, [loc[int(j)] for j in J], Ce)
+                np.add.at(Cb, np.searchsorted(nodes, J), Ce)
             G = Cb.conj().T @ (md_inv[nodes][:, None] * Cb)
             dSinv = np.linalg.solve(np.eye(npj) + sysd.dS[b] @ G, sysd.dS[b].astype(dtype))
             P1 = Cb.conj().T @ (md_inv[nodes][:, None] * np.asarray(X[nodes]))
@@ -256,12 +293,9 @@ def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
             if op == "H":
                 return mask[J][:, None] * np.asarray(X[J]).astype(dtype)
             t = md_inv[J][:, None] * np.asarray(X[J]).astype(dtype)
-            pos = {int(j): i for i, j in enumerate(J)}
             for b, (nodes, Cb, Wb) in W.items():
-                hit = [(pos[int(j)], i) for i, j in enumerate(nodes) if int(j) in pos]
-                if hit:
-                    ii = np.array([h[0] for h in hit])
-                    kk = np.array([h[1] for h in hit])
+                ii, kk = rows_in(J, nodes)
+                if len(ii):
                     t[ii] -= md_inv[J[ii]][:, None] * (Cb[kk] @ Wb)
             return t
 
@@ -272,8 +306,9 @@ def apply_HSinv_rows(sysd, X, cells, op="HSinv"):
             hit = [(pos_in[int(j)], i) for i, j in enumerate(J) if int(j) in pos_in]
             if not hit:
                 continue
-            He = fe.hamiltonian_cell_matrix(mesh, sysd, c[0], c[1], c[2], kpt, ref)
-            Ye = He @ (T_rows(J) * mask[J][:, None])
+            if c not in He_of:
+                He_of[c] = fe.hamiltonian_cell_matrix(mesh, sysd, c[0], c[1], c[2], kpt, ref)
+            Ye = He_of[c] @ (T_rows(J) * mask[J][:, None])
             for (i0, i) in hit:
                 acc[i0] += Ye[i]
         for a in A0:
