@@ -215,6 +215,15 @@ pawfe_status pawfe_cheb_filter_host_set(pawfe_ctx* ctx, pawfe_prec prec, int m, 
                                         void* const* X_host, const double* const* lambda, const long* ld,
                                         const int* B, int nblk);
 
+/* Upper bound b_U of the spectrum of H S^-1approx, the operator the filter iterates (Alg. 1 steps 1-2, L243-L244; L179): k-step
+ * Lanczos on H S^-1approx in the inner product <x, y> = Re x^dagger S^-1approx y (in which it is self-adjoint), FP64, with the
+ * library's own applies; b_U = 1.02 (theta_max(T_k) + beta_k).  v0: DEVICE, start vector, M FP64 scalars of the context's kind
+ * (complex interleaved); Dirichlet wall rows are ignored.  bU: HOST out.  theta_max, beta_k, steps_done: HOST out, optional
+ * (largest Ritz value of the tridiagonal matrix, last off-diagonal, Lanczos steps taken: fewer than k on breakdown).
+ * 1 <= k <= 256.  Not a hot call: allocates five work vectors and synchronises once per step.  Needs keep_fp64. */
+pawfe_status pawfe_lanczos_bound(pawfe_ctx* ctx, int k, const void* v0, double* bU, double* theta_max, double* beta_k,
+                                 int* steps_done);
+
 /* Column 2-norms ||x_i||_2, i < B, accumulated in FP64 (L290).  X: device, element type by prec;
  * out: DEVICE, B doubles. */
 pawfe_status pawfe_col_norms(pawfe_ctx* ctx, pawfe_prec prec, const void* X, long ld, int B, double* out);

@@ -73,13 +73,16 @@ def scaled_chebyshev(x, m, b0, bW, bU):
     return T((np.asarray(x) - c) / e) / T((b0 - c) / e)
 
 
-def lanczos_upper_bound(apply_H, apply_Sinv, M, k=10, seed=0, dtype=float, mask=None):
+def lanczos_upper_bound(apply_H, apply_Sinv, M, k=10, seed=0, dtype=float, mask=None, v0=None):
     """Upper bound b_U of the spectrum of the iterated operator H S^-1approx (same spectrum as
     S^-1approx H; Alg. 1 steps 1-2; reading R17).  k-step Lanczos in the
     S^-1approx inner product <x,y> = x^dagger S^-1approx y, in which H S^-1approx is self-adjoint;
-    b_U = 1.02 * (theta_max + beta_k)."""
-    rng = np.random.default_rng(seed)
-    v = rng.standard_normal((M, 1)).astype(dtype)
+    b_U = 1.02 * (theta_max + beta_k).  v0: optional start vector (default: seeded standard normal)."""
+    if v0 is None:
+        rng = np.random.default_rng(seed)
+        v = rng.standard_normal((M, 1)).astype(dtype)
+    else:                                   # start vector given (the random numbers the method draws are passed in)
+        v = np.array(v0, dtype=dtype).reshape(M, 1)
     if mask is not None:
         v = v * mask[:, None]
     ip = lambda x, y: np.real(np.vdot(x, apply_Sinv(y)))

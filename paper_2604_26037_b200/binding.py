@@ -28,7 +28,7 @@ SYMBOLS = [
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
-    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read",
+    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read", "pawfe_lanczos_bound",
 ]
 
 
@@ -84,6 +84,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_cell_timing.argtypes = [vp, C.c_int]
     lib.pawfe_cell_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
     lib.pawfe_setup_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
+    lib.pawfe_lanczos_bound.argtypes = [vp, C.c_int, vp, dp, dp, dp, ip]
     lib.pawfe_cell_kernel_name.argtypes = [vp, C.c_int, C.c_int]
     lib.pawfe_cell_kernel_name.restype = C.c_char_p
     for s in SYMBOLS:
@@ -289,6 +290,14 @@ class Context:
         bv = (C.c_int * n)(*[int(x) for x in Bs])
         self._check(self.lib.pawfe_cheb_filter_host_set(self._h, int(prec), int(m), float(b0), float(bW), float(bU),
                                                         xs, ls, ldv, bv, n), "pawfe_cheb_filter_host_set")
+
+    def lanczos_bound(self, k: int, v0):
+        """b_U of H S^-1approx from a k-step Lanczos started at the FP64 device vector v0 (pawfe_lanczos_bound).
+        Returns (bU, theta_max, beta_k, steps)."""
+        bU, th, bk, st = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+        self._check(self.lib.pawfe_lanczos_bound(self._h, int(k), self._ptr(v0), C.byref(bU), C.byref(th), C.byref(bk), C.byref(st)),
+                    "pawfe_lanczos_bound")
+        return bU.value, th.value, bk.value, st.value
 
     def col_norms(self, prec: int, X, ld: int, B: int, out):
         self._check(self.lib.pawfe_col_norms(self._h, int(prec), self._ptr(X), int(ld), int(B), self._ptr(out)),

@@ -9,6 +9,7 @@
 #include "apply_impl.h"
 #include "setup_fp64.cuh"
 #include "nonlocal_f32.cuh"
+#include "ptx_sm100.cuh"
 #include "kernels_stream.cuh"
 #include <algorithm>
 #include <cmath>
@@ -25,6 +26,8 @@ struct FusedPlan {
   float* d_GD = nullptr;        // [nnb][npj][npj]:  G^{ab} Delta^b_Sinv
   int* d_cps = nullptr;         // [ncell + 1] cell -> its (cell, atom) pairs
   int* d_cpi = nullptr;         // [npairs] pair indices by cell
+  int* d_pcells = nullptr; int npcells = 0;   // cells that have at least one pair (grid of k_proj_cell)
+  bool proj_cell = false;       // projection kernel: cell-parallel (k_proj_cell) or pair-parallel (k_proj2 / k_projF)
   int ext_ksteps = 4;
   // scratch for block width <= Bcap
   int Bcap = 0; long ldw = 0;
@@ -262,6 +265,109 @@ k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// (ii) partial non-local projection, CELL-parallel:  Ppart[pair][al][v] = sum_I C^{e,a}[I][al] X[J(e,I)][v]  for every pair of
+//   the cell.  One CTA per (cell that has pairs, tile of 64 real columns): the cell's rows are brought to shared memory ONCE
+//   (cp.async, 16 bytes per thread and row piece) and every pair of the cell is projected from there -- the pair-parallel
+//   k_proj2 / k_projF read the rows once per pair (config 4: 40k pairs on 33k cells, 14 GB per step instead of 7 GB).
+//   256 threads = 16 row groups x 16 column quads; the row groups are summed in a fixed order (shuffle, then warp by warp in
+//   shared memory), so the per-pair partials are bit-reproducible; k_psum adds them pair by pair.
+//   CPLX: interleaved (re, im) columns, Cd complex [pair][NPJ][n][2].  dynamic smem: see proj_cell_smem().
+// ------------------------------------------------------------------------------------------------
+constexpr int kPcVT = 64;   // real columns per CTA
+template <int NPJ, bool CPLX>
+__global__ void __launch_bounds__(256, 2)
+k_proj_cell(MeshDev md, const int* __restrict__ pcells, const int* __restrict__ cps, const int* __restrict__ cpi,
+            const float* __restrict__ Cd, const float* __restrict__ X, long ldx, int Wr, float* __restrict__ Ppart, long ldp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int cw = CPLX ? 2 : 1;
+  const int n = md.n, n1 = md.n1;
+  float* tile = reinterpret_cast<float*>(smem_raw);                         // [n][64]
+  float* Cs = tile + (size_t)n * kPcVT;                                     // [NPJ][n][cw]
+  float* red = Cs;                                                          // [4][NPJ][64], reuses Cs once a pair's FMAs are done
+  const int e = pcells[blockIdx.x];
+  const int v0 = blockIdx.y * kPcVT;
+  int cx, cy, cz;
+  mesh_cell_coords(md, e, &cx, &cy, &cz);
+  // rows -> shared memory (Dirichlet wall rows and columns beyond the block: zero fill)
+  const uint32_t tile_a = ptx::smem_u32(tile);
+  for (int i = threadIdx.x; i < n * (kPcVT / 4); i += 256) {
+    const int I = i >> 4, q = i & 15;
+    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+    const long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+    const bool ok = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] != 0.0 && v0 + 4 * q < Wr;
+    ptx::cp_async16(tile_a + (uint32_t)(I * kPcVT + 4 * q) * 4, ok ? X + J * ldx + v0 + 4 * q : X, ok ? 16u : 0u);
+  }
+  ptx::cp_async_commit();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int vq = threadIdx.x & 15, rg = threadIdx.x >> 4;   // column quad, row group (rows rg, rg + 16, ...)
+  for (int q = cps[e]; q < cps[e + 1]; ++q) {
+    const int pr = cpi[q];
+    __syncthreads();   // everyone is done with Cs / red of the previous pair
+    for (int i = threadIdx.x; i < NPJ * n * cw; i += 256) Cs[i] = Cd[(long)pr * NPJ * n * cw + i];
+    ptx::cp_async_wait<0>();
+    __syncthreads();
+    float4 acc[NPJ];
+#pragma unroll
+    for (int al = 0; al < NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int I = rg; I < n; I += 16) {
+      const float4 x = *reinterpret_cast<const float4*>(&tile[I * kPcVT + 4 * vq]);
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) {
+        if (CPLX) {
+          const float2 cv = *reinterpret_cast<const float2*>(&Cs[(al * n + I) * 2]);
+          acc[al].x = fmaf(cv.x, x.x, acc[al].x); acc[al].x = fmaf(-cv.y, x.y, acc[al].x);
+          acc[al].y = fmaf(cv.x, x.y, acc[al].y); acc[al].y = fmaf(cv.y, x.x, acc[al].y);
+          acc[al].z = fmaf(cv.x, x.z, acc[al].z); acc[al].z = fmaf(-cv.y, x.w, acc[al].z);
+          acc[al].w = fmaf(cv.x, x.w, acc[al].w); acc[al].w = fmaf(cv.y, x.z, acc[al].w);
+        } else {
+          const float cv = Cs[al * n + I];
+          acc[al].x = fmaf(cv, x.x, acc[al].x); acc[al].y = fmaf(cv, x.y, acc[al].y);
+          acc[al].z = fmaf(cv, x.z, acc[al].z); acc[al].w = fmaf(cv, x.w, acc[al].w);
+        }
+      }
+    }
+    // the warp's two row groups (lanes l and l ^ 16), then warp w + 4 onto warp w, then the four sums in order
+#pragma unroll
+    for (int al = 0; al < NPJ; ++al) {
+      acc[al].x += __shfl_xor_sync(0xffffffffu, acc[al].x, 16); acc[al].y += __shfl_xor_sync(0xffffffffu, acc[al].y, 16);
+      acc[al].z += __shfl_xor_sync(0xffffffffu, acc[al].z, 16); acc[al].w += __shfl_xor_sync(0xffffffffu, acc[al].w, 16);
+    }
+    __syncthreads();   // all reads of Cs are done: red may overwrite it
+    if (w >= 4 && lane < 16) {
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) *reinterpret_cast<float4*>(&red[((w - 4) * NPJ + al) * kPcVT + 4 * vq]) = acc[al];
+    }
+    __syncthreads();
+    if (w < 4 && lane < 16) {
+#pragma unroll
+      for (int al = 0; al < NPJ; ++al) {
+        float4* r4 = reinterpret_cast<float4*>(&red[(w * NPJ + al) * kPcVT + 4 * vq]);
+        const float4 u = *r4;
+        *r4 = make_float4(acc[al].x + u.x, acc[al].y + u.y, acc[al].z + u.z, acc[al].w + u.w);
+      }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NPJ * 16; i += 256) {
+      const int al = i >> 4, qq = i & 15;
+      if (v0 + 4 * qq < Wr) {
+        float4 t = *reinterpret_cast<const float4*>(&red[al * kPcVT + 4 * qq]);
+#pragma unroll
+        for (int ww = 1; ww < 4; ++ww) {
+          const float4 u = *reinterpret_cast<const float4*>(&red[(ww * NPJ + al) * kPcVT + 4 * qq]);
+          t.x += u.x; t.y += u.y; t.z += u.z; t.w += u.w;
+        }
+        *reinterpret_cast<float4*>(Ppart + ((long)pr * NPJ + al) * ldp + v0 + 4 * qq) = t;
+      }
+    }
+  }
+  ptx::cp_async_wait<0>();
+}
+template <int NPJ, bool CPLX>
+size_t proj_cell_smem(int n) {
+  return ((size_t)n * kPcVT + std::max(((size_t)NPJ * n * (CPLX ? 2 : 1) + 3) / 4 * 4, (size_t)4 * NPJ * kPcVT)) * sizeof(float);
+}
+
 // P[a][al][.] = sum over the atom's pairs, in pair order, of the per-pair partial projections (k_proj2 / k_projF with Ppart):
 // the ordered replacement of their cross-CTA reductions.  grid = (natoms * npj, ceil(Wq / 128)), block = 128; Wq = quads
 // of 4 real columns that hold data; ldq = leading dimension / 4.
@@ -432,7 +538,7 @@ k_recover_ordered(MeshDev md, const int* __restrict__ cps, const int* __restrict
 void free_plan(FusedPlan* p) {
   if (!p) return;
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
-  cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD); cudaFree(p->d_cps); cudaFree(p->d_cpi);
+  cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD); cudaFree(p->d_cps); cudaFree(p->d_cpi); cudaFree(p->d_pcells);
   cudaFree(p->d_P1); cudaFree(p->d_Ppart); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
   cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
   if (p->aux) cudaStreamDestroy(p->aux);
@@ -457,6 +563,14 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
   {
     std::vector<int> fill(cps.begin(), cps.end() - 1);
     for (long q = 0; q < c->npairs; ++q) cpi[fill[pc[q]]++] = (int)q;
+  }
+  {
+    std::vector<int> pcs;
+    for (int e = 0; e < ncell; ++e) if (cps[e + 1] > cps[e]) pcs.push_back(e);
+    p->npcells = (int)pcs.size();
+    if (!pcs.empty()) TRY(upload(c, &p->d_pcells, pcs));
+    p->proj_cell = p->npcells > 0 && (double)c->npairs / p->npcells >= 1.8;
+    if (const char* d = getenv("PAWFE_PROJ")) p->proj_cell = p->npcells > 0 && d[0] == 'c';
   }
   // K-extension entries: every cell sharing a node with a pair cell of the atom (the pair cells and their 26 neighbours)
   std::vector<std::vector<int>> cell_atoms(ncell);
@@ -599,18 +713,7 @@ pawfe_status ensure_block(pawfe_ctx* c, FusedPlan* p, float** buf, size_t* have,
   return PAWFE_OK;
 }
 
-// P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple)
-template <int NPJ>
-pawfe_status project_cplx(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int Wr) {
-  const int n = c->n;
-  const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)NPJ * n * 2 + 3) / 4 * 16 + (size_t)NPJ * 128 * 4;
-  TRY(pawfe_ensure_smem(c, (const void*)k_projF<NPJ, true>, smem));
-  k_projF<NPJ, true><<<dim3((unsigned)c->npairs, ceil_div(Wr, 128)), 256, smem, c->stream>>>(
-      c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw, p->d_Ppart);
-  KERNEL_CHECK(c, "k_projF");
-  return PAWFE_OK;
-}
-
+// P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple).
 // X: the block as floats (complex: interleaved), ldx in floats; B vectors.
 pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
   if (c->npairs == 0) return PAWFE_OK;
@@ -623,13 +726,53 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
     KERNEL_CHECK(c, "k_psum");
     return PAWFE_OK;
   };
-  if (c->cplx) {
+  // Projection into per-pair partials.  Cell-parallel (rows staged once per cell) where the cells that have pairs hold about
+  // two or more (config 4: 2.07 pairs per such cell, 6.0 ms against 7.65 ms per step); pair-parallel streaming otherwise
+  // (configs 1 / 2 / 3: 1.39 / 1.52 / 1.36 pairs per cell, 0.29 / 3.15 / 1.76 ms against 0.40 / 3.97 / 1.72 ms;
+  // profiles/r02_projection_kernels.md).  PAWFE_PROJ=cell|pair overrides (read once, at plan creation).
+  const int Wr = B * (c->cplx ? 2 : 1);
+  if (!p->proj_cell) {
+    const dim3 grid((unsigned)c->npairs, ceil_div(Wr, 128));
+    if (c->cplx) {
+      const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)npj * n * 2 + 3) / 4 * 16 + (size_t)npj * 128 * 4;
+#define CASE_PF(N) case N: TRY(pawfe_ensure_smem(c, (const void*)k_projF<N, true>, smem)); \
+      k_projF<N, true><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw, p->d_Ppart); break;
+      switch (npj) {
+        CASE_PF(1) CASE_PF(2) CASE_PF(3) CASE_PF(4) CASE_PF(5) CASE_PF(6) CASE_PF(7) CASE_PF(8)
+        CASE_PF(9) CASE_PF(10) CASE_PF(11) CASE_PF(12) CASE_PF(13) CASE_PF(14) CASE_PF(15) CASE_PF(16)
+      }
+#undef CASE_PF
+      KERNEL_CHECK(c, "k_projF");
+    } else {
+      const size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4;
+#define CASE_P2(N) case N: TRY(pawfe_ensure_smem(c, (const void*)k_proj2<N>, smem)); \
+      k_proj2<N><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw, p->d_Ppart); break;
+      switch (npj) {
+        CASE_P2(1) CASE_P2(2) CASE_P2(3) CASE_P2(4) CASE_P2(5) CASE_P2(6) CASE_P2(7) CASE_P2(8)
+        CASE_P2(9) CASE_P2(10) CASE_P2(11) CASE_P2(12) CASE_P2(13) CASE_P2(14) CASE_P2(15) CASE_P2(16)
+      }
+#undef CASE_P2
+      KERNEL_CHECK(c, "k_proj2");
+    }
+  } else if (p->npcells > 0) {
+    const dim3 grid((unsigned)p->npcells, ceil_div(Wr, kPcVT));
+#define LAUNCH_PC(N, CP)                                                                                                   \
+    do {                                                                                                                    \
+      const size_t smem = proj_cell_smem<N, CP>(n);                                                                         \
+      TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell<N, CP>, smem));                                                     \
+      k_proj_cell<N, CP><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, (const float*)c->d_Cd32, X, \
+                                                          ldx, Wr, p->d_Ppart, p->ldw);                                     \
+    } while (0)
+#define CASE_PC(N) case N: if (c->cplx) LAUNCH_PC(N, true); else LAUNCH_PC(N, false); break;
     switch (npj) {
-#define CASE_PC(N) case N: TRY(project_cplx<N>(c, p, X, ldx, 2 * B)); break;
       CASE_PC(1) CASE_PC(2) CASE_PC(3) CASE_PC(4) CASE_PC(5) CASE_PC(6) CASE_PC(7) CASE_PC(8)
       CASE_PC(9) CASE_PC(10) CASE_PC(11) CASE_PC(12) CASE_PC(13) CASE_PC(14) CASE_PC(15) CASE_PC(16)
-#undef CASE_PC
     }
+#undef CASE_PC
+#undef LAUNCH_PC
+    KERNEL_CHECK(c, "k_proj_cell");
+  }
+  if (c->cplx) {
     TRY(psum(2 * B));
     const int Bpad = (int)(roundup4(2 * B) / 2);
     k_couple<float2><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(
@@ -638,23 +781,6 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
     KERNEL_CHECK(c, "k_couple");
     return PAWFE_OK;
   }
-  size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4;
-  dim3 grid((unsigned)c->npairs, ceil_div(B, 128));
-#define LAUNCH_PROJ2(NPJ)                                                                                            \
-  do {                                                                                                               \
-    TRY(pawfe_ensure_smem(c, (const void*)k_proj2<NPJ>, smem)); \
-    k_proj2<NPJ><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw, p->d_Ppart); \
-  } while (0)
-  switch (npj) {
-    case 1: LAUNCH_PROJ2(1); break;   case 2: LAUNCH_PROJ2(2); break;   case 3: LAUNCH_PROJ2(3); break;
-    case 4: LAUNCH_PROJ2(4); break;   case 5: LAUNCH_PROJ2(5); break;   case 6: LAUNCH_PROJ2(6); break;
-    case 7: LAUNCH_PROJ2(7); break;   case 8: LAUNCH_PROJ2(8); break;   case 9: LAUNCH_PROJ2(9); break;
-    case 10: LAUNCH_PROJ2(10); break; case 11: LAUNCH_PROJ2(11); break; case 12: LAUNCH_PROJ2(12); break;
-    case 13: LAUNCH_PROJ2(13); break; case 14: LAUNCH_PROJ2(14); break; case 15: LAUNCH_PROJ2(15); break;
-    default: LAUNCH_PROJ2(16); break;
-  }
-#undef LAUNCH_PROJ2
-  KERNEL_CHECK(c, "k_proj2");
   TRY(psum(B));
   const int Bpad = (int)roundup4(B);
   k_couple<float><<<dim3(c->natoms, ceil_div(Bpad, kCoupleLanes)), kCoupleLanes * npj, 0, c->stream>>>(

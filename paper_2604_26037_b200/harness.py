@@ -1,6 +1,5 @@
 """Harness around the filter: the steps of Algorithm 1 that are NOT on the hot path
-this library builds -- S-orthonormalisation, Rayleigh-Ritz (steps 4-6), the upper spectral bound (step 1),
-residual norms (L290) -- written with torch dense linear algebra on the device around the library's own
+this library builds -- S-orthonormalisation, Rayleigh-Ritz (steps 4-6), residual norms (L290) -- written with torch dense linear algebra on the device around the library's own
 H / S / S^-1approx applications.  They exist so that tests and bench.py can drive the filter with the
 inputs Algorithm 2 expects (an S-orthonormal Ritz block, its Ritz values, [b0, bW, bU]).
 section 8(f) lists moving them into the library as NEXT-1 / NEXT-2.
@@ -73,30 +72,12 @@ class Harness:
 
     def upper_bound(self, k: int = 10, seed: int = 0) -> float:
         """b_U for the iterated operator H S^-1approx: k-step Lanczos in the S^-1approx inner product,
-        b_U = 1.02 (theta_max + beta_k) (reading R17)."""
+        b_U = 1.02 (theta_max + beta_k) (reading R17), inside the library (pawfe_lanczos_bound); only the
+        seeded start vector is drawn here."""
         g = torch.Generator(device="cpu").manual_seed(seed)
         shape = (self.M, 1, 2) if self.cplx else (self.M, 1)
         v = torch.randn(shape, dtype=torch.float64, generator=g).cuda()
-        ip = lambda x, y: float(self.gram(x, self.apply("Sinv", y)).real.item())
-        # zero the Dirichlet boundary rows: S^-1approx v is zero there, so use it as the mask
-        mask = (self.apply("Sinv", torch.ones_like(v)).abs().sum(dim=tuple(range(1, v.dim()))) > 0).to(v.dtype)
-        v = v * mask.reshape((-1,) + (1,) * (v.dim() - 1))
-        v = v / np.sqrt(ip(v, v))
-        vprev = torch.zeros_like(v)
-        beta = 0.0
-        alphas, betas = [], []
-        for _ in range(k):
-            w = self.apply("H", self.apply("Sinv", v)) - beta * vprev
-            alpha = ip(v, w)
-            w = w - alpha * v
-            beta = float(np.sqrt(max(ip(w, w), 0.0)))
-            alphas.append(alpha)
-            betas.append(beta)
-            if beta < 1e-14:
-                break
-            vprev, v = v, w / beta
-        T = np.diag(alphas) + np.diag(betas[:-1], 1) + np.diag(betas[:-1], -1)
-        return 1.02 * (np.linalg.eigvalsh(T)[-1] + betas[-1])
+        return self.ctx.lanczos_bound(k, v)[0]
 
 
 def cast_block(X64: torch.Tensor, prec: int) -> torch.Tensor:

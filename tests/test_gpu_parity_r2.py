@@ -320,3 +320,29 @@ def test_full_loop_eigenvalues_twins(name, prec):
     assert err < 1e-6, (name, prec, err)
     res = hz.residual_norms(X, lam)[:12]
     assert np.max(res) < 1e-3, (name, prec, res)                          # L290's per-SCF rule is 1e-2
+
+
+# ---- generalised Lanczos bound in the library ---------------------------------------------------
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1_twin", "cfg3_twin", "cfg4_twin"])
+def test_lanczos_bound_in_library(name):
+    """pawfe_lanczos_bound (Alg. 1 step 1, L243; reading R17) against oracle.chfsi.lanczos_upper_bound from the SAME start
+    vector: the k = 10 bound, and on config 0 a true upper bound of the dense spectrum of S^-1approx H."""
+    from oracle import chfsi
+    cfg, sysd, ops, ctx = _setup(name)
+    rng = np.random.default_rng(cfg.seed + 99)
+    v0 = rng.standard_normal(ops.mesh.M) + (1j * rng.standard_normal(ops.mesh.M) if cfg.complex else 0.0)
+    want = chfsi.lanczos_upper_bound(ops.apply_H, ops.apply_Sinv, ops.mesh.M, k=10, dtype=ops.dtype, mask=ops.mask, v0=v0)
+    vd = to_dev(v0.reshape(-1, 1), "fp64", cfg.complex)
+    bU, theta, beta, steps = ctx.lanczos_bound(10, vd)
+    assert steps == 10
+    assert abs(bU - want) < 1e-9 * abs(want), (name, bU, want)
+    assert abs(bU - 1.02 * (theta + beta)) < 1e-12 * abs(bU)
+    if name == "cfg0":
+        lam_max = np.max(np.real(np.linalg.eigvals(ops.apply_Sinv(ops.dense_H()))))
+        assert bU >= lam_max
+    # garbage in Dirichlet wall rows of the start vector is ignored
+    if cfg.bc == "dirichlet":
+        v1 = v0.copy()
+        v1[~ops.mask] = 1e6
+        assert abs(ctx.lanczos_bound(10, to_dev(v1.reshape(-1, 1), "fp64", cfg.complex))[0] - bU) < 1e-9 * abs(bU)
