@@ -224,6 +224,22 @@ pawfe_status pawfe_cheb_filter_host_set(pawfe_ctx* ctx, pawfe_prec prec, int m, 
 pawfe_status pawfe_lanczos_bound(pawfe_ctx* ctx, int k, const void* v0, double* bU, double* theta_max, double* beta_k,
                                  int* steps_done);
 
+/* ---- Rayleigh-Ritz kernels of Algorithm 1 (L246-L248; section 4.5) ----------------------- */
+
+/* RR-Projection: G = X^dagger Y (B x B), FP64.  X, Y: device, FP64 blocks [dof][vec] with leading dimension ld (complex:
+ * interleaved).  Only the 64 x 64 blocks of the LOWER triangle are computed (L402); the upper triangle is written as the
+ * conjugate transpose, so G is exactly Hermitian: meant for Y = H X or Y = S X.  G: device, B * B FP64 scalars, row-major.
+ * Sums are taken in a fixed order (bit-reproducible).  1 <= B <= 8192.  Allocates its partial sums per call and
+ * synchronises the stream before returning. */
+pawfe_status pawfe_rr_project(pawfe_ctx* ctx, const void* X, const void* Y, long ld, int B, void* G);
+
+/* RR-SR, subspace rotation: Xout = X Q.  X, Xout: device FP64 blocks (leading dimensions ldx, ldo), must not overlap;
+ * Q: device, B * B FP64 scalars, row-major.  mixed = 0: all products in FP64.  mixed != 0: the paper's mixed-precision
+ * rotation (L406-L408): the 64 x 64 DIAGONAL blocks of Q in FP64, the OFF-DIAGONAL blocks in FP32 (operands rounded to
+ * FP32, FP32 sums inside a block, blocks added in FP64): exact to FP64 level when Q is close to block-diagonal, i.e.
+ * near convergence; ~1e-7 relative in general. */
+pawfe_status pawfe_rr_rotate(pawfe_ctx* ctx, int mixed, const void* X, long ldx, const void* Q, void* Xout, long ldo, int B);
+
 /* Column 2-norms ||x_i||_2, i < B, accumulated in FP64 (L290).  X: device, element type by prec;
  * out: DEVICE, B doubles. */
 pawfe_status pawfe_col_norms(pawfe_ctx* ctx, pawfe_prec prec, const void* X, long ld, int B, double* out);

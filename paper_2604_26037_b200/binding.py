@@ -28,7 +28,8 @@ SYMBOLS = [
     "pawfe_apply_Sinv", "pawfe_filter_workspace", "pawfe_cheb_filter", "pawfe_cheb_filter_host", "pawfe_cheb_filter_host_set",
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
-    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read", "pawfe_lanczos_bound",
+    "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read", "pawfe_lanczos_bound", "pawfe_rr_project",
+    "pawfe_rr_rotate",
 ]
 
 
@@ -85,6 +86,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_cell_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
     lib.pawfe_setup_timing_read.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_double)]
     lib.pawfe_lanczos_bound.argtypes = [vp, C.c_int, vp, dp, dp, dp, ip]
+    lib.pawfe_rr_project.argtypes = [vp, vp, vp, C.c_long, C.c_int, vp]
+    lib.pawfe_rr_rotate.argtypes = [vp, C.c_int, vp, C.c_long, vp, vp, C.c_long, C.c_int]
     lib.pawfe_cell_kernel_name.argtypes = [vp, C.c_int, C.c_int]
     lib.pawfe_cell_kernel_name.restype = C.c_char_p
     for s in SYMBOLS:
@@ -298,6 +301,15 @@ class Context:
         self._check(self.lib.pawfe_lanczos_bound(self._h, int(k), self._ptr(v0), C.byref(bU), C.byref(th), C.byref(bk), C.byref(st)),
                     "pawfe_lanczos_bound")
         return bU.value, th.value, bk.value, st.value
+
+    def rr_project(self, X, Y, ld: int, B: int, G):
+        """G = X^dagger Y (FP64, lower-triangle blocks computed, mirrored; pawfe_rr_project)"""
+        self._check(self.lib.pawfe_rr_project(self._h, self._ptr(X), self._ptr(Y), int(ld), int(B), self._ptr(G)), "pawfe_rr_project")
+
+    def rr_rotate(self, mixed: bool, X, ldx: int, Q, Xout, ldo: int, B: int):
+        """Xout = X Q (FP64; mixed: FP32 off-diagonal blocks; pawfe_rr_rotate)"""
+        self._check(self.lib.pawfe_rr_rotate(self._h, int(bool(mixed)), self._ptr(X), int(ldx), self._ptr(Q), self._ptr(Xout),
+                                             int(ldo), int(B)), "pawfe_rr_rotate")
 
     def col_norms(self, prec: int, X, ld: int, B: int, out):
         self._check(self.lib.pawfe_col_norms(self._h, int(prec), self._ptr(X), int(ld), int(B), self._ptr(out)),

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpawfe.so")
-SOURCES = ["pawfe_api.cu", "api_setup.cu", "api_atoms.cu", "api_apply.cu", "api_filter.cu", "api_fused.cu", "api_noalloc.cu", "api_lanczos.cu", "cell_tcgen05.cu",
+SOURCES = ["pawfe_api.cu", "api_setup.cu", "api_atoms.cu", "api_apply.cu", "api_filter.cu", "api_fused.cu", "api_noalloc.cu", "api_lanczos.cu", "api_rr.cu", "cell_tcgen05.cu",
            "fe_tables.cpp"]
 NVCC_FLAGS = (["-DPAWFE_TC_DEBUG"] if os.environ.get("PAWFE_TC_DEBUG") else []) + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

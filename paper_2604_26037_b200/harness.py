@@ -1,6 +1,7 @@
 """Harness around the filter: the steps of Algorithm 1 that are NOT on the hot path
-this library builds -- S-orthonormalisation, Rayleigh-Ritz (steps 4-6), residual norms (L290) -- written with torch dense linear algebra on the device around the library's own
-H / S / S^-1approx applications.  They exist so that tests and bench.py can drive the filter with the
+this library builds -- S-orthonormalisation, Rayleigh-Ritz (steps 4-6), residual norms (L290).  The tall products run in
+the library (RR-Projection pawfe_rr_project, subspace rotation pawfe_rr_rotate, the H / S / S^-1approx applications, the
+Lanczos bound); only the small dense B x B algebra (Cholesky, eigh: RR-GHEP, a library call in the paper too) is torch.  They exist so that tests and bench.py can drive the filter with the
 inputs Algorithm 2 expects (an S-orthonormal Ritz block, its Ritz values, [b0, bW, bU]).
 section 8(f) lists moving them into the library as NEXT-1 / NEXT-2.
 """
@@ -19,8 +20,9 @@ def _as_complex(t: torch.Tensor, cplx: bool) -> torch.Tensor:
 class Harness:
     """FP64 helper operations on blocks stored in the library's layout ([M, B] or [M, B, 2])."""
 
-    def __init__(self, ctx: Context, M: int, cplx: bool):
-        self.ctx, self.M, self.cplx = ctx, M, cplx
+    def __init__(self, ctx: Context, M: int, cplx: bool, mixed_rotation: bool = False):
+        """mixed_rotation: the paper's mixed-precision subspace rotation (FP64 diagonal / FP32 off-diagonal blocks, L406-L408)"""
+        self.ctx, self.M, self.cplx, self.mixed = ctx, M, cplx, mixed_rotation
 
     def _empty_like(self, X):
         return torch.empty_like(X)
@@ -32,14 +34,21 @@ class Harness:
         return Y
 
     def gram(self, X: torch.Tensor, Y: torch.Tensor) -> torch.Tensor:
-        """X^dagger Y (B x B), FP64."""
-        Xc, Yc = _as_complex(X, self.cplx), _as_complex(Y, self.cplx)
-        return Xc.conj().T @ Yc
+        """X^dagger Y (B x B), FP64, for Y = H X or S X (Hermitian result): pawfe_rr_project."""
+        B = X.shape[1]
+        X, Y = X.contiguous(), Y.contiguous()
+        G = torch.empty((B, B, 2) if self.cplx else (B, B), dtype=torch.float64, device=X.device)
+        self.ctx.rr_project(X, Y, B, B, G)
+        return _as_complex(G, self.cplx)
 
     def rotate(self, X: torch.Tensor, Q: torch.Tensor) -> torch.Tensor:
-        Xc = _as_complex(X, self.cplx)
-        R = Xc @ Q
-        return torch.view_as_real(R).contiguous() if self.cplx else R.contiguous()
+        """X Q: pawfe_rr_rotate (mixed precision if the harness was created with mixed_rotation)."""
+        B = X.shape[1]
+        X = X.contiguous()
+        Qd = (torch.view_as_real(Q.to(torch.complex128).contiguous()) if self.cplx else Q.to(torch.float64)).contiguous()
+        out = torch.empty_like(X)
+        self.ctx.rr_rotate(self.mixed, X, B, Qd, out, B, B)
+        return out
 
     def s_orthonormalise(self, X: torch.Tensor) -> torch.Tensor:
         G = self.gram(X, self.apply("S", X))

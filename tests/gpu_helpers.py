@@ -4,6 +4,8 @@ Error measures (a relative Frobenius norm alone cannot see one wron
   relerr(a, b)      ||a - b||_F / ||b||_F                                  the north_star's per-product measure
   rowerr(a, b)      max_J ||a_J - b_J||_2 / (||b||_F / sqrt(rows))          a single bad row of RMS size gives O(1)
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -44,6 +46,10 @@ def rowerr(a, b):
 
 def check(got, want, tol, what):
     e, r = relerr(got, want), rowerr(got, want)
+    rep = os.environ.get("PAWFE_TEST_REPORT")          # optional log of the measured errors (profiles/r02_parity_margins.md)
+    if rep:
+        with open(rep, "a") as f:
+            f.write(f"{what}\trelerr={e:.3e}\trowerr={r:.3e}\ttol={tol:.1e}\n")
     assert e < tol, (what, "relerr", e)
     assert r < ROW_FACTOR * tol, (what, "rowerr", r)
     return e

@@ -146,7 +146,7 @@ def test_filter_call(name, prec):
     torch.cuda.synchronize()
     got = _to_host(Xd, cfg.complex)
     err = _relerr(got, want)
-    tol = {"fp64": 1e-10, "fp32": 5e-4, "tf32": 5e-2}[prec]
+    tol = {"fp64": 1e-10, "fp32": 5e-5, "tf32": 1e-2}[prec]
     assert err < tol, (name, prec, err)
 
 
@@ -250,7 +250,7 @@ def test_filter_ragged_block_width(B):
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, False), want) < 5e-2
+    assert _relerr(_to_host(Xd, False), want) < 1e-2
 
 
 @pytest.mark.parametrize("name,B", [("cfg2_twin", 136), ("cfg3_twin", 80), ("cfg4_twin", 256)])
@@ -285,7 +285,7 @@ def test_filter_wide_blocks(name, B):
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, cfg.complex), want) < 5e-2
+    assert _relerr(_to_host(Xd, cfg.complex), want) < 1e-2
 
 
 def test_filter_complex_odd_width_generic_sequence():
@@ -306,7 +306,7 @@ def test_filter_complex_odd_width_generic_sequence():
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, True), want) < 5e-2
+    assert _relerr(_to_host(Xd, True), want) < 1e-2
 
 
 @pytest.mark.parametrize("name,prec", [("cfg1_twin", "fp32"), ("cfg3_twin", "tf32"), ("cfg0", "fp64")])
@@ -332,7 +332,7 @@ def test_filter_host_block_set(name, prec):
     host = [_to_dev(X, prec, cfg.complex).cpu().pin_memory() for X in Xs]
     dev = [h.cuda() for h in host]
     ctx.cheb_filter_host_set(PREC[prec], m, b0, bW, bU, [h.data_ptr() for h in host], lams, widths, widths)
-    tol = {"fp64": 1e-10, "fp32": 5e-4, "tf32": 5e-2}[prec]
+    tol = {"fp64": 1e-10, "fp32": 5e-5, "tf32": 1e-2}[prec]
     for k, B in enumerate(widths):
         got = _to_host(host[k], cfg.complex)
         assert _relerr(got, wants[k]) < tol, (name, prec, k, _relerr(got, wants[k]))
@@ -340,7 +340,10 @@ def test_filter_host_block_set(name, prec):
         ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
         ctx.cheb_filter(PREC[prec], m, b0, bW, bU, dev[k], lams[k], B, B, ws, nbytes)
         torch.cuda.synchronize()
-        # same kernels on the same data: equal up to the order of the FP32 assembly reductions (R20)
+        # same kernels on the same data.  FP32 storage: the ordered path is bit-reproducible except for the FP64 residual set-up,
+        # whose FP64 atomics can move the last bit of the FP32 R_Y (1e-7 level after m steps).  FP64 mode: the FP64 assembly is
+        # by atomics whose order differs from run to run: ~1e-15 per product, amplified by the degree-4 recurrence (the gate
+        # was 1e-13 before commit 61383d5, which a run with an unlucky atomic order exceeded; 1e-12 = the per-product bar)
         assert _relerr(_to_host(dev[k], cfg.complex), got) < (1e-12 if prec == "fp64" else 1e-5)
 
 
@@ -388,7 +391,7 @@ def test_single_vector_block(name):
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, 1, 1, ws, nbytes)
     torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, False), want) < 5e-2
+    assert _relerr(_to_host(Xd, False), want) < 1e-2
 
 
 def test_maximum_block_width():
@@ -415,7 +418,7 @@ def test_maximum_block_width():
     ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
     ctx.cheb_filter(TF32, m, b0, bW, bU, Xd, lam, B, B, ws, nbytes)
     torch.cuda.synchronize()
-    assert _relerr(_to_host(Xd, False), wantf) < 5e-2
+    assert _relerr(_to_host(Xd, False), wantf) < 1e-2
 
 
 def test_error_behaviour():
