@@ -24,6 +24,7 @@ template <> struct Acc<false> {
   static __device__ __forceinline__ double zero() { return 0.0; }
   static __device__ __forceinline__ double conj(double a) { return a; }
   static __device__ __forceinline__ double add(double a, double b) { return a + b; }
+  static __device__ __forceinline__ double real_part(double a) { return a; }
 };
 template <> struct Acc<true> {
   typedef double2 T;
@@ -36,6 +37,7 @@ template <> struct Acc<true> {
   static __device__ __forceinline__ double2 zero() { return make_double2(0.0, 0.0); }
   static __device__ __forceinline__ double2 conj(double2 a) { return make_double2(a.x, -a.y); }
   static __device__ __forceinline__ double2 add(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+  static __device__ __forceinline__ double2 real_part(double2 a) { return make_double2(a.x, 0.0); }
 };
 
 // partial[slab][tile][i][j] = sum over the slab's rows J of conj(X[J][ib kT + i]) Y[J][jb kT + j], lower tiles (ib >= jb) only.
@@ -97,6 +99,7 @@ __global__ void k_rr_reduce(int ntiles, int nslab, int B, const typename Acc<CPL
     T s = Acc<CPLX>::zero();
     for (int sl = 0; sl < nslab; ++sl) s = Acc<CPLX>::add(s, partial[((long)sl * ntiles + blockIdx.x) * kT * kT + e]);
     if (ib == jb && j > i) continue;               // diagonal tile: keep its lower part, mirrored below
+    if (i == j) s = Acc<CPLX>::real_part(s);         // a Hermitian matrix has a real diagonal (the sum is real only to rounding)
     G[(long)i * B + j] = s;
     if (i != j) G[(long)j * B + i] = Acc<CPLX>::conj(s);
   }

@@ -45,7 +45,7 @@ class Harness:
         """X Q: pawfe_rr_rotate (mixed precision if the harness was created with mixed_rotation)."""
         B = X.shape[1]
         X = X.contiguous()
-        Qd = (torch.view_as_real(Q.to(torch.complex128).contiguous()) if self.cplx else Q.to(torch.float64)).contiguous()
+        Qd = (torch.view_as_real(Q.to(torch.complex128).resolve_conj().contiguous()) if self.cplx else Q.to(torch.float64)).contiguous()
         out = torch.empty_like(X)
         self.ctx.rr_rotate(self.mixed, X, B, Qd, out, B, B)
         return out

@@ -392,7 +392,7 @@ def test_rr_projection_and_rotation(name, B):
     Qn = np.eye(B) + 1e-6 * Qr                                                  # near convergence: off-diagonal blocks are tiny
     ctx.rr_rotate(True, Xd, B, to_dev(Qn, "fp64", cfg.complex), out, B, B)
     torch.cuda.synchronize()
-    assert relerr(to_host(out, cfg.complex), X @ Qn) < 1e-12
+    assert relerr(to_host(out, cfg.complex), X @ Qn) < 1e-11          # off-diagonal blocks: 1e-6 of Q at FP32 accuracy
     # one Rayleigh-Ritz step through the harness (library projection + rotation, torch for the B x B pencil)
     hz = Harness(ctx, ops.mesh.M, cfg.complex)
     _, lam = hz.rayleigh_ritz(Xd)
