@@ -57,9 +57,10 @@ typedef enum {
 
 /* Arithmetic of the cell contraction (section 4.4; L11, L27 for TF32):
  *   FP64: every step in double (reference mode).
- *   FP32: FP32 storage, FP32-accurate arithmetic inside H S^-1approx.  Real contexts run the cell contraction on
- *         tcgen05 tensor cores as three TF32 passes on operands split into the part kind::tf32 keeps and the rest
- *         (hi*hi + lo*hi + hi*lo, FP32 accumulation; ~1e-6 relative per product); complex contexts use FP32 FMAs.
+ *   FP32: FP32 storage, FP32-accurate arithmetic inside H S^-1approx.  The cell contraction runs on tcgen05 tensor cores
+ *         as three TF32 passes on operands split into the part kind::tf32 keeps and the rest (hi*hi + lo*hi + hi*lo,
+ *         FP32 accumulation; ~1e-6 relative per product), real and complex contexts alike; blocks that do not meet the
+ *         tensor-core path's alignment rules use FP32 FMAs.
  *   TF32: FP32 storage; operands of the cell contraction truncated to TF32 inside tcgen05 tensor
  *         cores, FP32 accumulation (~7e-4 relative per product).  Nothing else is TF32. */
 typedef enum { PAWFE_FP64 = 0, PAWFE_FP32 = 1, PAWFE_TF32 = 2 } pawfe_prec;

@@ -352,7 +352,7 @@ extern "C" pawfe_status pawfe_apply_HSinv(pawfe_ctx* c, pawfe_prec prec, const v
 extern "C" const char* pawfe_cell_kernel_name(const pawfe_ctx* c, pawfe_prec prec, int B) {
   if (!c) return "none";
   if (prec == PAWFE_FP64) return "dmma_fp64";
-  if (prec == PAWFE_FP32) return (!c->cplx && tc_supported(c, B)) ? "tcgen05_3xtf32" : "simt_fp32";
+  if (prec == PAWFE_FP32) return tc_supported(c, B) ? "tcgen05_3xtf32" : "simt_fp32";
   if (tc_supported(c, B)) return "tcgen05_tf32";
   return "simt_tf32_emulated";
 }

@@ -839,7 +839,7 @@ void fused_invalidate(pawfe_ctx* c) {
 }
 
 bool fused_supported(pawfe_ctx* c, pawfe_prec prec, int B) {
-  return (prec == PAWFE_TF32 || (prec == PAWFE_FP32 && !c->cplx)) && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
+  return (prec == PAWFE_TF32 || prec == PAWFE_FP32) && c->have_h64 && c->have_atoms && tc_supported(c, B) && 2 * c->npj <= 32;
 }
 
 // run work on the plan's auxiliary stream, ordered after everything enqueued so far on the context's stream

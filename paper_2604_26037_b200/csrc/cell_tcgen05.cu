@@ -232,6 +232,7 @@ k_cell_tcgen05(const TcArgs a) {
     }
   }
   const uint64_t pol_stream = ptx::policy_evict_first();   // data read once per launch: cell-matrix blocks, residual source
+  const uint64_t pol_keep = ptx::policy_evict_last();      // the rows of Y: written first, then added to by up to 7 later cells
 
   uint32_t st_s = 0, st_ph = 0;   // running stage index and phase of this role's walk over the ring (same sequence in every role)
   uint32_t sub_iter = 0;          // running subtile counter: accumulator buffer = sub_iter & 1
@@ -311,7 +312,7 @@ k_cell_tcgen05(const TcArgs a) {
               for (int i = 0; i < 4; ++i) {
                 const int k = sub + 4 * i;
                 const long e = k < nq ? eJ[col0 + k] : 2;
-                if (!(e & 2)) ptx::red_add_v4(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[k * 32 + v4]));
+                if (!(e & 2)) { if (TC_DBG(a, 2048)) ptx::red_add_v4(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[k * 32 + v4])); else ptx::red_add_v4_hint(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[k * 32 + v4]), pol_keep); }
               }
             }
             __syncwarp();
@@ -340,7 +341,7 @@ k_cell_tcgen05(const TcArgs a) {
               for (int i = 0; i < 8; ++i) {
                 const int q = sub + 4 * i;
                 const long e = q < nq ? eJ[col0 + q] : 2;
-                if (!(e & 2)) ptx::red_add_v4(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[q * 32 + v4]));
+                if (!(e & 2)) { if (TC_DBG(a, 2048)) ptx::red_add_v4(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[q * 32 + v4])); else ptx::red_add_v4_hint(reinterpret_cast<float*>(yv + (e & ~15L)), *reinterpret_cast<const float4*>(&stg[q * 32 + v4]), pol_keep); }
               }
             }
             __syncwarp();
@@ -612,7 +613,7 @@ k_cell_tcgen05(const TcArgs a) {
             o.y = (float)((double)(-a.ac * ry.y - a.zz1 * rx.y) + ya.y * l[1]);
             o.z = (float)((double)(-a.ac * ry.z - a.zz1 * rx.z) + yb.x * l[2]);
             o.w = (float)((double)(-a.ac * ry.w - a.zz1 * rx.w) + yb.y * l[3]);
-            if (!TC_DBG(a, 128)) ptx::stg_f4(yg + ((long)rows[kBrWarps * i] << 4), o);
+            if (!TC_DBG(a, 128)) { if (TC_DBG(a, 2048)) ptx::stg_f4(yg + ((long)rows[kBrWarps * i] << 4), o); else ptx::stg_f4_hint(yg + ((long)rows[kBrWarps * i] << 4), o, pol_keep); }
           }
           __syncwarp();                                // every lane has read the slot before it is refilled
           issue(i + kBrSlots);

@@ -62,7 +62,7 @@ def test_bit_identical_twice(name, B):
     """No unordered floating-point reduction is left on the FP32-storage path: the cell kernel assembles in the plan's cell
     order (cell_tcgen05.cu), projections are summed pair by pair (k_psum), recovery is owner-computes (k_recover_ordered).
     Two runs of H X, of H S^-1approx X and of a filter call fed with H Psi, S Psi (pawfe_cheb_filter_hs) give the same BITS,
-    in TF32 and FP32 (3xTF32) modes, one-CTA and CTA-pair kernels, real / complex / Dirichlet.
+    in TF32 and FP32 (3xTF32) modes, one-CTA and CTA-pair kernels, real / complex / Dirichlet (complex FP32 included).
     pawfe_cheb_filter's own FP64 residual set-up assembles with FP64 atomics (order-dependent at 1e-16, which can move the
     last bit of the FP32 R_Y): its two runs agree to 1e-6 of the block norm, not bitwise."""
     from paper_2604_26037_b200 import PREC
@@ -71,8 +71,7 @@ def test_bit_identical_twice(name, B):
     b0, bW, bU = bounds(ops, lam)
     ld = B + (B % 2 if cfg.complex else (-B) % 4)
     Ba = B - B % 4          # the applies take the tensor-core path for widths that are multiples of 4 (ragged widths: SIMT + atomics)
-    # complex FP32 mode is the SIMT sequence (atomic assembly): the ordered path is TF32 there
-    for prec in (("tf32",) if cfg.complex else ("tf32", "fp32")):
+    for prec in ("tf32", "fp32"):
         Xp = np.zeros((X.shape[0], ld), dtype=X.dtype)
         Xp[:, :B] = X
         Xd = to_dev(Xp, prec, cfg.complex)
