@@ -299,10 +299,11 @@ def run_own(args):
         # one pinned host copy of the block set per call (warm-up + e2e_steps): never filter a host block twice in place
         host_sets = [[x.cpu().pin_memory() for x in ring[0]] for _ in range(1 + e2e_steps)]
     else:
-        # cycled resident blocks: two pinned SOURCE blocks and two pinned WORK blocks; a helper thread refills the next work
-        # block from its source while the current one is filtered (in place) -- the host-side refill is not part of the path
+        # cycled resident blocks: two pinned SOURCE blocks and two PAIRS of pinned WORK blocks; each call filters one pair in
+        # place (copies of the pair's second block run under the first block's filter) while a helper thread refills the
+        # other pair from the sources -- the host-side refill is not part of the path
         src = [ring[0][k].cpu().pin_memory() for k in range(2)]
-        work = [torch.empty_like(src[0]).pin_memory() for _ in range(2)]
+        work = [[torch.empty_like(src[0]).pin_memory() for _ in range(2)] for _ in range(2)]
     del ring, blocks, ws, scratch  # the host-buffer call owns its own device block and workspace
     torch.cuda.empty_cache()
 
@@ -314,14 +315,20 @@ def run_own(args):
 
     def e2e_pass_cycled(nb):
         import threading
-        work[0].copy_(src[0])
-        for b in range(nb):
+
+        def refill(pair):
+            for q in range(2):
+                work[pair][q].copy_(src[q])
+        refill(0)
+        for b0_ in range(0, nb, 2):
+            pair = (b0_ // 2) % 2
             t = None
-            if b + 1 < nb:
-                t = threading.Thread(target=lambda q=(b + 1) % 2: work[q].copy_(src[q]))
+            if b0_ + 2 < nb:
+                t = threading.Thread(target=refill, args=(1 - pair,))
                 t.start()
-            w = widths[b % nblk]
-            ctx.cheb_filter_host(prec, m, b0, bW, bU, work[b % 2].data_ptr(), lams[b % 2][:w], B, w)
+            ws_ = [widths[(b0_ + q) % nblk] for q in range(min(2, nb - b0_))]
+            ctx.cheb_filter_host_set(prec, m, b0, bW, bU, [work[pair][q].data_ptr() for q in range(len(ws_))],
+                                     [lams[q][:w] for q, w in enumerate(ws_)], [B] * len(ws_), ws_)
             if t is not None:
                 t.join()
 
@@ -398,7 +405,7 @@ def run_own(args):
         "clocks": clocks,
         "e2e": {"value": world * units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nblk * blk_bytes,
                 "d2h_bytes_per_step": nblk * blk_bytes, "steps": e2e_steps,
-                "how": "pawfe_cheb_filter_host per block (two pinned work blocks refilled by a helper thread)" if cycled
+                "how": "pawfe_cheb_filter_host_set on pairs of pinned work blocks (refilled by a helper thread between calls)" if cycled
                        else "pawfe_cheb_filter_host_set (copies pipelined under the filters)"},
         "gpu_launches": launches,
         "roofline": roof,
