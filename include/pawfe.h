@@ -127,6 +127,12 @@ pawfe_status pawfe_get_pairs(pawfe_ctx* ctx, int* pair_cell, int* pair_atom);
  * Synchronises the host. */
 pawfe_status pawfe_set_projector_blocks(pawfe_ctx* ctx, const double* Cd, int is_device);
 
+/* Which G^a enters Delta^a_Sinv = (dS^a^-1 + G^a)^-1 of Eq. 29 (L225-L228): variant 0 (default) G^a = C^a^dagger M_D^-1 C^a
+ * (exact Woodbury inverse of M_D + C dS C^dagger for one atom); variant 1 the paper's cheaper alternative (text after Eq. 29,
+ * L228) G^a ~ <p_alpha|p_beta>, the overlap matrix of the projector functions (mesh-independent; radial quadrature on the
+ * host).  Recomputes Delta_Sinv; pawfe_atoms_create resets the variant to 0.  Synchronises the host. */
+pawfe_status pawfe_set_sinv_variant(pawfe_ctx* ctx, int variant);
+
 /* Replace D (Delta_H changes every SCF step, Eq. 18).  host, natoms*nproj*nproj. */
 pawfe_status pawfe_update_coupling(pawfe_ctx* ctx, const double* D);
 

@@ -28,5 +28,6 @@ Round 2 (tests/test_oracle_pins_r2.py; each verified to turn red under the mutat
   k-term of H^e .............. k with three different components, per-axis +-G plane waves (G_x <-> G_z swap)
   operators.apply_H_rows ..... == rows of the assembled product on config 0, complex and Dirichlet twins (dropped cell)
   operators.apply_HSinv_rows . == rows of apply_H(apply_Sinv(X)) on the same cases (atom reached through a neighbour cell)
+  paw.projector_overlap_matrix == brute-force 3-D Gram matrix of the projector functions (the <p|p> variant of L228)
 With these, no function on the path is "parity unpinned".
 """

@@ -14,7 +14,8 @@ from . import fe, paw
 
 
 class PawOperators:
-    def __init__(self, sysd, with_potential: bool = True, with_nonlocal: bool = True):
+    def __init__(self, sysd, with_potential: bool = True, with_nonlocal: bool = True, sinv_variant: int = 0):
+        """sinv_variant: 0 = G^a = C^a^dagger M_D^-1 C^a in Eq. 29 (default); 1 = G^a = <p_alpha|p_beta>"""
         cfg = sysd.cfg
         self.sysd = sysd
         self.cfg = cfg
@@ -44,7 +45,8 @@ class PawOperators:
         self.Ch = self.C.conj().T.tocsr()
         self.Dbig = paw.block_diag_coupling(self.D)
         self.dSbig = paw.block_diag_coupling(self.dS)
-        self.dSinv, self.G = paw.sinv_couplings(self.C, self.md_inv, self.dS)
+        self.dSinv, self.G = paw.sinv_couplings(self.C, self.md_inv, self.dS,
+                                                paw.projector_overlap_matrix(sysd) if sinv_variant == 1 else None)
         self.dSinvbig = paw.block_diag_coupling(self.dSinv)
 
     # -- cell matrices ---------------------------------------------------------------------

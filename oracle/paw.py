@@ -117,16 +117,35 @@ def block_diag_coupling(blocks: np.ndarray):
     return sp.block_diag([sp.csr_matrix(b) for b in blocks], format="csr")
 
 
-def sinv_couplings(C, md_inv: np.ndarray, dS: np.ndarray):
+def projector_overlap_matrix(sysd) -> np.ndarray:
+    """<p_alpha|p_beta> = int p_alpha(d) p_beta(d) d^3d over the cutoff sphere: the matrix the paper says C^a^dagger M^-1 C^a
+    "can be approximated by" (text after Eq. 29, PAPER.md:L228).  Real orthonormal Y_lm make it block diagonal in (l, m);
+    the radial integral is taken by adaptive quadrature."""
+    import scipy.integrate as si
+    npj = len(sysd.proj_l)
+    O = np.zeros((npj, npj))
+    for a in range(npj):
+        for b in range(npj):
+            if sysd.proj_l[a] != sysd.proj_l[b] or sysd.proj_m[a] != sysd.proj_m[b]:
+                continue
+            l, sa, sb, rc = int(sysd.proj_l[a]), sysd.proj_sigma[a], sysd.proj_sigma[b], sysd.rc
+            f = lambda r: (r ** l * math.exp(-r * r / (2 * sa * sa)) * (1 - (r / rc) ** 2) ** 2) * \
+                          (r ** l * math.exp(-r * r / (2 * sb * sb)) * (1 - (r / rc) ** 2) ** 2) * r * r
+            O[a, b] = sysd.proj_amp[a] * sysd.proj_amp[b] * si.quad(f, 0.0, rc, epsabs=1e-14, epsrel=1e-13)[0]
+    return O
+
+
+def sinv_couplings(C, md_inv: np.ndarray, dS: np.ndarray, G_override=None):
     """Delta^a_Sinv = (dS^a^-1 + C^a^dagger M_D^-1 C^a)^-1   (Eq. 29), evaluated as
     (I + dS^a G^a)^-1 dS^a (reading R10: same matrix, no inverse of dS^a).  Cross-atom blocks of
-    C^dagger M_D^-1 C are dropped (approximation (ii))."""
+    C^dagger M_D^-1 C are dropped (approximation (ii)).  G_override: use this n_pj x n_pj matrix as G^a of every atom
+    instead (the <p_alpha|p_beta> variant of L228: projector_overlap_matrix)."""
     natoms, npj, _ = dS.shape
     out = np.zeros((natoms, npj, npj), dtype=C.dtype)
     G = []
     for a in range(natoms):
         Ca = C[:, a * npj:(a + 1) * npj]
-        Ga = (Ca.conj().T @ sp.diags(md_inv) @ Ca).toarray()
+        Ga = (Ca.conj().T @ sp.diags(md_inv) @ Ca).toarray() if G_override is None else np.asarray(G_override, dtype=C.dtype)
         G.append(Ga)
         out[a] = np.linalg.solve(np.eye(npj) + dS[a] @ Ga, dS[a].astype(C.dtype))
     return out, np.array(G)

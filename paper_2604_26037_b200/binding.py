@@ -29,7 +29,7 @@ SYMBOLS = [
     "pawfe_col_norms", "pawfe_launch_count", "pawfe_cell_kernel_name", "pawfe_cell_timing",
     "pawfe_cell_timing_read", "pawfe_set_cell_matrices", "pawfe_get_pairs", "pawfe_set_projector_blocks",
     "pawfe_apply_HSinv", "pawfe_prepare", "pawfe_cheb_filter_hs", "pawfe_apply_Sinv_noalloc", "pawfe_setup_timing_read", "pawfe_lanczos_bound", "pawfe_rr_project",
-    "pawfe_rr_rotate",
+    "pawfe_rr_rotate", "pawfe_set_sinv_variant",
 ]
 
 
@@ -68,6 +68,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.pawfe_get_pairs.argtypes = [vp, ip, ip]
     lib.pawfe_set_projector_blocks.argtypes = [vp, vp, C.c_int]
     lib.pawfe_prepare.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+    lib.pawfe_set_sinv_variant.argtypes = [vp, C.c_int]
     lib.pawfe_cheb_filter_hs.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp, dp,
                                          C.c_long, C.c_int, vp, C.c_size_t]
     for f in (lib.pawfe_apply_H, lib.pawfe_apply_S, lib.pawfe_apply_Sinv, lib.pawfe_apply_HSinv, lib.pawfe_apply_Sinv_noalloc):
@@ -188,6 +189,10 @@ class Context:
 
     def prepare(self, prec: int, Bmax: int, mmax: int):
         self._check(self.lib.pawfe_prepare(self._h, int(prec), int(Bmax), int(mmax)), "pawfe_prepare")
+
+    def set_sinv_variant(self, variant: int):
+        """0: G^a = C^dagger M_D^-1 C (Eq. 29); 1: G^a = <p_alpha|p_beta> (L228)."""
+        self._check(self.lib.pawfe_set_sinv_variant(self._h, int(variant)), "pawfe_set_sinv_variant")
 
     def update_coupling(self, D):
         D = _f64(D)

@@ -141,7 +141,7 @@ extern "C" pawfe_status pawfe_atoms_create(pawfe_ctx* c, int natoms, const doubl
       if (!(rc < 0.5 * c->box[d])) { c->err = "rc must be < box/2 for periodic meshes"; return PAWFE_EINVAL; }
   CUDA_TRY(c, cudaSetDevice(c->device));
   pawfe_free_atoms(c);
-  c->natoms = natoms; c->npj = nproj; c->rc = rc;
+  c->natoms = natoms; c->npj = nproj; c->rc = rc; c->sinv_variant = 0;
   c->pos.assign(pos, pos + 3 * (size_t)natoms);
   c->proj_l.assign(proj_l, proj_l + nproj); c->proj_m.assign(proj_m, proj_m + nproj);
   c->proj_sigma.assign(proj_sigma, proj_sigma + nproj); c->proj_amp.assign(proj_amp, proj_amp + nproj);
@@ -228,6 +228,35 @@ extern "C" pawfe_status pawfe_atoms_create(pawfe_ctx* c, int natoms, const doubl
   return PAWFE_OK;
 }
 
+namespace {
+// G^a of the variant in force (same for every atom in variant 1): natoms*npj*npj*cw doubles
+//   variant 1 (text after Eq. 29): C^a^dagger M^-1 C^a ~ <p_alpha|p_beta> = int p_alpha p_beta d^3x
+//     = delta_ll' delta_mm' amp amp' int_0^rc r^(2l) exp(-r^2/2s^2) exp(-r^2/2s'^2) (1-(r/rc)^2)^4 r^2 dr   (orthonormal Y_lm),
+//     by a 96-point Gauss-Legendre rule on [0, rc].
+std::vector<double> sinv_G(const pawfe_ctx* c) {
+  if (c->sinv_variant == 0) return c->h_G;
+  const int npj = c->npj, cw = c->cplx ? 2 : 1;
+  std::vector<double> x, w, O((size_t)npj * npj, 0.0);
+  gauss_legendre_rule(96, x, w);
+  for (int a = 0; a < npj; ++a)
+    for (int b = 0; b < npj; ++b) {
+      if (c->proj_l[a] != c->proj_l[b] || c->proj_m[a] != c->proj_m[b]) continue;
+      double s = 0.0;
+      for (size_t q = 0; q < x.size(); ++q) {
+        const double r = 0.5 * c->rc * (x[q] + 1.0), cut = 1.0 - (r / c->rc) * (r / c->rc);
+        const double f = std::pow(r, 2 * c->proj_l[a]) * std::exp(-r * r / (2 * c->proj_sigma[a] * c->proj_sigma[a])) *
+                         std::exp(-r * r / (2 * c->proj_sigma[b] * c->proj_sigma[b])) * cut * cut * cut * cut * r * r;
+        s += 0.5 * c->rc * w[q] * f;
+      }
+      O[(size_t)a * npj + b] = c->proj_amp[a] * c->proj_amp[b] * s;
+    }
+  std::vector<double> G((size_t)c->natoms * npj * npj * cw, 0.0);
+  for (int at = 0; at < c->natoms; ++at)
+    for (size_t i = 0; i < (size_t)npj * npj; ++i) G[((size_t)at * npj * npj + i) * cw] = O[i];
+  return G;
+}
+}  // namespace
+
 extern "C" pawfe_status pawfe_get_pairs(pawfe_ctx* c, int* pair_cell, int* pair_atom) {
   if (!c || !pair_cell || !pair_atom) return PAWFE_EINVAL;
   if (!c->have_atoms) return PAWFE_ESTATE;
@@ -259,7 +288,19 @@ extern "C" pawfe_status pawfe_set_projector_blocks(pawfe_ctx* c, const double* C
   }
   c->h_G = G;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  return pawfe_upload_couplings(c, nullptr, c->h_dS.data(), G);
+  return pawfe_upload_couplings(c, nullptr, c->h_dS.data(), sinv_G(c));
+}
+
+// Which G^a enters Delta^a_Sinv = (dS^a^-1 + G^a)^-1 (Eq. 29): recomputes Delta_Sinv and drops the fused plan.
+extern "C" pawfe_status pawfe_set_sinv_variant(pawfe_ctx* c, int variant) {
+  if (!c) return PAWFE_EINVAL;
+  if (variant != 0 && variant != 1) { c->err = "S^-1approx variant must be 0 or 1"; return PAWFE_EINVAL; }
+  if (!c->have_atoms) { c->err = "atoms not created"; return PAWFE_ESTATE; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  fused_invalidate(c);
+  c->sinv_variant = variant;
+  return pawfe_upload_couplings(c, nullptr, c->h_dS.data(), sinv_G(c));
 }
 
 extern "C" pawfe_status pawfe_update_coupling(pawfe_ctx* c, const double* D) {
@@ -267,7 +308,7 @@ extern "C" pawfe_status pawfe_update_coupling(pawfe_ctx* c, const double* D) {
   if (!c->have_atoms) return PAWFE_ESTATE;
   CUDA_TRY(c, cudaSetDevice(c->device));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  return pawfe_upload_couplings(c, D, c->h_dS.data(), c->h_G);
+  return pawfe_upload_couplings(c, D, c->h_dS.data(), sinv_G(c));
 }
 
 extern "C" pawfe_status pawfe_get_sinv_coupling(pawfe_ctx* c, double* out) {

@@ -27,7 +27,6 @@ struct FusedPlan {
   int* d_cps = nullptr;         // [ncell + 1] cell -> its (cell, atom) pairs
   int* d_cpi = nullptr;         // [npairs] pair indices by cell
   int* d_pcells = nullptr; int npcells = 0;   // cells that have at least one pair (grid of k_proj_cell)
-  bool proj_cell = false;       // projection kernel: cell-parallel (k_proj_cell) or pair-parallel (k_proj2 / k_projF)
   int ext_ksteps = 4;
   // scratch for block width <= Bcap
   int Bcap = 0; long ldw = 0;
@@ -185,126 +184,70 @@ k_build_ext(MeshDev md, const int* __restrict__ ext_cell, const int* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
-// (ii) partial non-local projection, pair-parallel:  P[a][al][v] += sum_I C^{e,a}[I][al] X[J(e,I)][v]
-//   grid = (npairs, ceil(B/128)), block = 256 (8 warps over rows, lane = 4 consecutive vectors).
-//   dynamic smem: n longs + npj*n floats + 16*128 floats.  P must be zero on entry.
-// ------------------------------------------------------------------------------------------------
-template <int NPJ>
-__global__ void __launch_bounds__(256, (NPJ <= 9 ? 3 : 2))
-k_proj2(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom,
-        const float* __restrict__ Cd, const float* __restrict__ X, long ldx, int B,
-        float* __restrict__ P, long ldp, float* __restrict__ Ppart) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int n = md.n, n1 = md.n1;
-  long* nodeO = reinterpret_cast<long*>(smem_raw);     // byte offset of the node's row, -1: masked
-  float* Cs = reinterpret_cast<float*>(nodeO + (n + 1) / 2 * 2);     // [NPJ][n], 16-byte aligned
-  float* red = Cs + ((size_t)NPJ * n + 3) / 4 * 4;     // [NPJ][128], 16-byte aligned
-  const int pr = blockIdx.x, a = pair_atom[pr];
-  int cx, cy, cz;
-  mesh_cell_coords(md, pair_cell[pr], &cx, &cy, &cz);
-  for (int I = threadIdx.x; I < n; I += blockDim.x) {
-    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
-    long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-    nodeO[I] = (md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] == 0.0) ? -1 : J * ldx * 4;
-  }
-  for (int i = threadIdx.x; i < NPJ * n; i += blockDim.x) Cs[i] = Cd[(long)pr * NPJ * n + i];
-  for (int i = threadIdx.x; i < NPJ * 128; i += blockDim.x) red[i] = 0.f;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int v = blockIdx.y * 128 + lane * 4;
-  float4 acc[NPJ];
-#pragma unroll
-  for (int al = 0; al < NPJ; ++al) acc[al] = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (v < B) {
-    const char* xv = reinterpret_cast<const char*>(X + v);
-    // rows w, w + 8, ... ; four independent 16-byte loads in flight per thread before the first use
-    for (int I0 = w; I0 < n; I0 += 32) {
-      float4 x[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int I = I0 + 8 * u;
-        const long off = I < n ? nodeO[I] : -1;
-        x[u] = off >= 0 ? __ldg(reinterpret_cast<const float4*>(xv + off)) : make_float4(0.f, 0.f, 0.f, 0.f);
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int I = min(I0 + 8 * u, n - 1);   // x[u] is zero beyond n
-#pragma unroll
-        for (int al = 0; al < NPJ; ++al) {
-          const float cv = Cs[al * n + I];
-          acc[al].x = fmaf(cv, x[u].x, acc[al].x); acc[al].y = fmaf(cv, x[u].y, acc[al].y);
-          acc[al].z = fmaf(cv, x[u].z, acc[al].z); acc[al].w = fmaf(cv, x[u].w, acc[al].w);
-        }
-      }
-    }
-  }
-  // cross-warp sum in shared memory, one warp per round (fixed order; shared-memory float atomics are CAS loops)
-  for (int r = 0; r < 8; ++r) {
-    if (w == r && v < B) {
-#pragma unroll
-      for (int al = 0; al < NPJ; ++al) {
-        float4* q = reinterpret_cast<float4*>(red + al * 128 + lane * 4);
-        float4 t = *q;
-        t.x += acc[al].x; t.y += acc[al].y; t.z += acc[al].z; t.w += acc[al].w;
-        *q = t;
-      }
-    }
-    __syncthreads();
-  }
-  for (int i = threadIdx.x; i < NPJ * 32; i += blockDim.x) {
-    const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
-    if (vv < B) {
-      const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
-      if (Ppart) {   // this pair's partial projection; k_psum adds the atom's pairs in a fixed order (bit-reproducible)
-        *reinterpret_cast<float4*>(Ppart + ((long)pr * NPJ + al) * ldp + vv) = val;
-      } else {
-        float* dst = P + ((long)a * NPJ + al) * ldp + vv;
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
-      }
-    }
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
 // (ii) partial non-local projection, CELL-parallel:  Ppart[pair][al][v] = sum_I C^{e,a}[I][al] X[J(e,I)][v]  for every pair of
 //   the cell.  One CTA per (cell that has pairs, tile of 64 real columns): the cell's rows are brought to shared memory ONCE
-//   (cp.async, 16 bytes per thread and row piece) and every pair of the cell is projected from there -- the pair-parallel
-//   k_proj2 / k_projF read the rows once per pair (config 4: 40k pairs on 33k cells, 14 GB per step instead of 7 GB).
+//   (cp.async, 16 bytes per thread and row piece) and every pair of the cell is projected from there (a pair-parallel
+//   kernel reads the rows once per pair: config 4 has 45k pairs on 22k such cells, 16 GB per step instead of 8 GB).
 //   256 threads = 16 row groups x 16 column quads; the row groups are summed in a fixed order (shuffle, then warp by warp in
 //   shared memory), so the per-pair partials are bit-reproducible; k_psum adds them pair by pair.
 //   CPLX: interleaved (re, im) columns, Cd complex [pair][NPJ][n][2].  dynamic smem: see proj_cell_smem().
 // ------------------------------------------------------------------------------------------------
 constexpr int kPcVT = 64;   // real columns per CTA
+// floats reserved for a pair's block (plus the alignment shift, whole 16-byte pieces) or the reduction scratch, whichever is larger
+template <int NPJ, bool CPLX>
+__host__ __device__ constexpr size_t proj_cell_cs_floats(int n) {
+  return ((size_t)NPJ * (CPLX ? 2 : 1) * n + 3 + 3) / 4 * 4 > (size_t)4 * NPJ * kPcVT ? ((size_t)NPJ * (CPLX ? 2 : 1) * n + 3 + 3) / 4 * 4 : (size_t)4 * NPJ * kPcVT;
+}
 template <int NPJ, bool CPLX>
 __global__ void __launch_bounds__(256, 2)
 k_proj_cell(MeshDev md, const int* __restrict__ pcells, const int* __restrict__ cps, const int* __restrict__ cpi,
-            const float* __restrict__ Cd, const float* __restrict__ X, long ldx, int Wr, float* __restrict__ Ppart, long ldp) {
+            const float* __restrict__ Cd, long cd_total, const float* __restrict__ X, long ldx, int Wr, float* __restrict__ Ppart,
+            long ldp) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int cw = CPLX ? 2 : 1;
+  constexpr int kCnt = NPJ * cw;                                            // floats of a pair's block per node
   const int n = md.n, n1 = md.n1;
   float* tile = reinterpret_cast<float*>(smem_raw);                         // [n][64]
-  float* Cs = tile + (size_t)n * kPcVT;                                     // [NPJ][n][cw]
-  float* red = Cs;                                                          // [4][NPJ][64], reuses Cs once a pair's FMAs are done
+  float* Csraw = tile + (size_t)n * kPcVT;                                  // the pair's block [NPJ][n][cw], shifted by <= 3 floats (see below)
+  float* red = Csraw;                                                       // [4][NPJ][64], reuses the block's space once a pair's FMAs are done
+  long* nodeO = reinterpret_cast<long*>(Csraw + proj_cell_cs_floats<NPJ, CPLX>(n));   // [n] element offset of the node's row, -1: masked
   const int e = pcells[blockIdx.x];
   const int v0 = blockIdx.y * kPcVT;
-  int cx, cy, cz;
-  mesh_cell_coords(md, e, &cx, &cy, &cz);
+  {
+    int cx, cy, cz;
+    mesh_cell_coords(md, e, &cx, &cy, &cz);
+    for (int I = threadIdx.x; I < n; I += 256) {
+      int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+      const long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+      nodeO[I] = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] != 0.0 ? J * ldx : -1;
+    }
+  }
+  __syncthreads();
   // rows -> shared memory (Dirichlet wall rows and columns beyond the block: zero fill)
-  const uint32_t tile_a = ptx::smem_u32(tile);
+  const uint32_t tile_a = ptx::smem_u32(tile), cs_a = ptx::smem_u32(Csraw);
   for (int i = threadIdx.x; i < n * (kPcVT / 4); i += 256) {
     const int I = i >> 4, q = i & 15;
-    int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
-    const long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
-    const bool ok = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] != 0.0 && v0 + 4 * q < Wr;
-    ptx::cp_async16(tile_a + (uint32_t)(I * kPcVT + 4 * q) * 4, ok ? X + J * ldx + v0 + 4 * q : X, ok ? 16u : 0u);
+    const long off = nodeO[I];
+    const bool ok = off >= 0 && v0 + 4 * q < Wr;
+    ptx::cp_async16(tile_a + (uint32_t)(I * kPcVT + 4 * q) * 4, ok ? X + off + v0 + 4 * q : X, ok ? 16u : 0u);
   }
-  ptx::cp_async_commit();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int vq = threadIdx.x & 15, rg = threadIdx.x >> 4;   // column quad, row group (rows rg, rg + 16, ...)
   for (int q = cps[e]; q < cps[e + 1]; ++q) {
     const int pr = cpi[q];
-    __syncthreads();   // everyone is done with Cs / red of the previous pair
-    for (int i = threadIdx.x; i < NPJ * n * cw; i += 256) Cs[i] = Cd[(long)pr * NPJ * n * cw + i];
+    __syncthreads();   // everyone is done with the block / red of the previous pair
+    // the pair's block by 16-byte copies: a block starts at a multiple of 4 bytes only (n is odd), so the copy starts at the
+    // 16-byte boundary below it and the block is read from Csraw + sh; nothing is read beyond the end of the array
+    const long start = (long)pr * kCnt * n;
+    const int sh = (int)(start & 3);
+    const float* src = Cd + (start - sh);
+    const int cnt4 = (kCnt * n + sh + 3) / 4;
+    for (int i = threadIdx.x; i < cnt4; i += 256) {
+      const long left = cd_total - (start - sh) - 4L * i;                   // floats of the array from this piece on
+      ptx::cp_async16(cs_a + 16u * i, src + 4 * i, left >= 4 ? 16u : (uint32_t)(4 * left));
+    }
+    ptx::cp_async_commit();
+    const float* Cs = Csraw + sh;
     ptx::cp_async_wait<0>();
     __syncthreads();
     float4 acc[NPJ];
@@ -365,10 +308,10 @@ k_proj_cell(MeshDev md, const int* __restrict__ pcells, const int* __restrict__ 
 }
 template <int NPJ, bool CPLX>
 size_t proj_cell_smem(int n) {
-  return ((size_t)n * kPcVT + std::max(((size_t)NPJ * n * (CPLX ? 2 : 1) + 3) / 4 * 4, (size_t)4 * NPJ * kPcVT)) * sizeof(float);
+  return ((size_t)n * kPcVT + proj_cell_cs_floats<NPJ, CPLX>(n)) * sizeof(float) + (size_t)n * sizeof(long);
 }
 
-// P[a][al][.] = sum over the atom's pairs, in pair order, of the per-pair partial projections (k_proj2 / k_projF with Ppart):
+// P[a][al][.] = sum over the atom's pairs, in pair order, of the per-pair partial projections (k_proj_cell):
 // the ordered replacement of their cross-CTA reductions.  grid = (natoms * npj, ceil(Wq / 128)), block = 128; Wq = quads
 // of 4 real columns that hold data; ldq = leading dimension / 4.
 __global__ void __launch_bounds__(128)
@@ -569,8 +512,6 @@ pawfe_status build_plan(pawfe_ctx* c, FusedPlan* p) {
     for (int e = 0; e < ncell; ++e) if (cps[e + 1] > cps[e]) pcs.push_back(e);
     p->npcells = (int)pcs.size();
     if (!pcs.empty()) TRY(upload(c, &p->d_pcells, pcs));
-    p->proj_cell = p->npcells > 0 && (double)c->npairs / p->npcells >= 1.8;
-    if (const char* d = getenv("PAWFE_PROJ")) p->proj_cell = p->npcells > 0 && d[0] == 'c';
   }
   // K-extension entries: every cell sharing a node with a pair cell of the atom (the pair cells and their 26 neighbours)
   std::vector<std::vector<int>> cell_atoms(ncell);
@@ -726,42 +667,18 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
     KERNEL_CHECK(c, "k_psum");
     return PAWFE_OK;
   };
-  // Projection into per-pair partials.  Cell-parallel (rows staged once per cell) where the cells that have pairs hold about
-  // two or more (config 4: 2.07 pairs per such cell, 6.0 ms against 7.65 ms per step); pair-parallel streaming otherwise
-  // (configs 1 / 2 / 3: 1.39 / 1.52 / 1.36 pairs per cell, 0.29 / 3.15 / 1.76 ms against 0.40 / 3.97 / 1.72 ms;
-  // profiles/r02_projection_kernels.md).  PAWFE_PROJ=cell|pair overrides (read once, at plan creation).
+  // Cell-parallel projection into per-pair partials (every pair belongs to exactly one cell of the list).  It replaced round
+  // 1's pair-parallel k_proj2 / k_projF, which read a cell's rows once per pair (profiles/r02_projection_kernels.md: config 4
+  // 7.65 -> 4.53 ms per step, configs 1 / 2 / 3: 0.29 / 3.15 / 1.76 -> 0.27 / 2.59 / 1.24 ms).
   const int Wr = B * (c->cplx ? 2 : 1);
-  if (!p->proj_cell) {
-    const dim3 grid((unsigned)c->npairs, ceil_div(Wr, 128));
-    if (c->cplx) {
-      const size_t smem = (size_t)(n + 1) / 2 * 16 + (size_t)(n + 3) / 4 * 16 + ((size_t)npj * n * 2 + 3) / 4 * 16 + (size_t)npj * 128 * 4;
-#define CASE_PF(N) case N: TRY(pawfe_ensure_smem(c, (const void*)k_projF<N, true>, smem)); \
-      k_projF<N, true><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, Wr, 0, p->d_P1, p->ldw, p->d_Ppart); break;
-      switch (npj) {
-        CASE_PF(1) CASE_PF(2) CASE_PF(3) CASE_PF(4) CASE_PF(5) CASE_PF(6) CASE_PF(7) CASE_PF(8)
-        CASE_PF(9) CASE_PF(10) CASE_PF(11) CASE_PF(12) CASE_PF(13) CASE_PF(14) CASE_PF(15) CASE_PF(16)
-      }
-#undef CASE_PF
-      KERNEL_CHECK(c, "k_projF");
-    } else {
-      const size_t smem = (size_t)(n + 1) / 2 * 16 + ((size_t)npj * n + 3) / 4 * 16 + (size_t)npj * 128 * 4;
-#define CASE_P2(N) case N: TRY(pawfe_ensure_smem(c, (const void*)k_proj2<N>, smem)); \
-      k_proj2<N><<<grid, 256, smem, c->stream>>>(c->md, c->d_pair_cell, c->d_pair_atom, (const float*)c->d_Cd32, X, ldx, B, p->d_P1, p->ldw, p->d_Ppart); break;
-      switch (npj) {
-        CASE_P2(1) CASE_P2(2) CASE_P2(3) CASE_P2(4) CASE_P2(5) CASE_P2(6) CASE_P2(7) CASE_P2(8)
-        CASE_P2(9) CASE_P2(10) CASE_P2(11) CASE_P2(12) CASE_P2(13) CASE_P2(14) CASE_P2(15) CASE_P2(16)
-      }
-#undef CASE_P2
-      KERNEL_CHECK(c, "k_proj2");
-    }
-  } else if (p->npcells > 0) {
+  if (p->npcells > 0) {
     const dim3 grid((unsigned)p->npcells, ceil_div(Wr, kPcVT));
 #define LAUNCH_PC(N, CP)                                                                                                   \
     do {                                                                                                                    \
       const size_t smem = proj_cell_smem<N, CP>(n);                                                                         \
       TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell<N, CP>, smem));                                                     \
-      k_proj_cell<N, CP><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, (const float*)c->d_Cd32, X, \
-                                                          ldx, Wr, p->d_Ppart, p->ldw);                                     \
+      k_proj_cell<N, CP><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, (const float*)c->d_Cd32,        \
+                                                          (long)c->npairs * N * n * (CP ? 2 : 1), X, ldx, Wr, p->d_Ppart, p->ldw); \
     } while (0)
 #define CASE_PC(N) case N: if (c->cplx) LAUNCH_PC(N, true); else LAUNCH_PC(N, false); break;
     switch (npj) {

@@ -166,6 +166,7 @@ struct pawfe_ctx {
   void* d_Cd32 = nullptr;  // same, float / float2
   std::vector<double> h_dS;          // natoms*npj*npj real
   std::vector<double> h_G;           // natoms*npj*npj scalars: G^a = C^a^dagger M_D^-1 C^a
+  int sinv_variant = 0;              // which G^a enters Delta_Sinv (Eq. 29): 0 = C^a^dagger M_D^-1 C^a, 1 = <p_alpha|p_beta> (L228)
   std::vector<double> h_dSinv;       // natoms*npj*npj scalars: Delta^a_Sinv (Eq. 29)
   void* d_D64 = nullptr; void* d_dS64 = nullptr; void* d_dSinv64 = nullptr;  // [atom][npj][npj] scalar
   void* d_D32 = nullptr; void* d_dS32 = nullptr; void* d_dSinv32 = nullptr;

@@ -10,8 +10,7 @@
 template <int NPJ, bool CPLX>
 __global__ void __launch_bounds__(256, (NPJ <= 9 ? 3 : 2))
 k_projF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ pair_atom, const float* __restrict__ Cd,
-        const float* __restrict__ X, long ldx /*floats*/, int Wr, int in_scale, float* __restrict__ P, long ldp /*floats*/,
-        float* __restrict__ Ppart = nullptr /* per-pair partials [pair][NPJ][ldp] instead of reductions into P */) {
+        const float* __restrict__ X, long ldx /*floats*/, int Wr, int in_scale, float* __restrict__ P, long ldp /*floats*/) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int cw = CPLX ? 2 : 1;
   const int n = md.n, n1 = md.n1;
@@ -86,12 +85,8 @@ k_projF(MeshDev md, const int* __restrict__ pair_cell, const int* __restrict__ p
     const int al = i >> 5, vv = blockIdx.y * 128 + (i & 31) * 4;
     if (vv < Wr) {
       const float4 val = *reinterpret_cast<const float4*>(&red[al * 128 + (i & 31) * 4]);
-      if (Ppart) {
-        *reinterpret_cast<float4*>(Ppart + ((long)pr * NPJ + al) * ldp + vv) = val;
-      } else {
-        float* dst = P + ((long)a * NPJ + al) * ldp + vv;
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
-      }
+      float* dst = P + ((long)a * NPJ + al) * ldp + vv;
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(val.x), "f"(val.y), "f"(val.z), "f"(val.w) : "memory");
     }
   }
 }

@@ -397,3 +397,44 @@ def test_rr_projection_and_rotation(name, B):
     _, lam = hz.rayleigh_ritz(Xd)
     _, lam_or = chfsi.rayleigh_ritz(ops.apply_H, ops.apply_S, X)
     assert np.max(np.abs(np.asarray(lam) - lam_or)) < 1e-9 * max(1.0, np.abs(lam_or).max())
+
+
+# ---- the <p|p> variant of Eq. 29 -------------------------------------------------
+
+@pytest.mark.parametrize("name", ["cfg2_twin", "cfg3_twin"])
+def test_sinv_projector_overlap_variant(name):
+    """pawfe_set_sinv_variant(1): Delta_Sinv built with G^a = <p_alpha|p_beta> instead of C^dagger M_D^-1 C, against the oracle's
+    operators built the same way: couplings, S^-1approx X, H S^-1approx X (fused kernels) and one filter call; variant 0 again
+    restores the default couplings."""
+    from oracle import chfsi
+    from oracle.operators import PawOperators
+    from paper_2604_26037_b200 import FP64, TF32, context_from_system
+    cfg, sysd, ops0, _ = _setup(name)
+    need_gpu()
+    ops = PawOperators(sysd, sinv_variant=1)
+    ctx = context_from_system(sysd, device=0, stream=torch.cuda.current_stream().cuda_stream)
+    try:
+        ctx.set_sinv_variant(1)
+        assert relerr(ctx.get_sinv_coupling(cfg.natoms, cfg.nproj), ops.dSinv) < 1e-9
+        assert relerr(ops.dSinv, ops0.dSinv) > 1e-3                                    # the variant is a different matrix
+        B, m = cfg.block, cfg.degree
+        X, lam = ritz_block(ops, cfg, B, stream=95)
+        Xd = to_dev(X, "fp64", cfg.complex)
+        Y = torch.empty_like(Xd)
+        ctx.apply_Sinv(FP64, Xd, Y, B, B)
+        torch.cuda.synchronize()
+        check(to_host(Y, cfg.complex), ops.apply_Sinv(X) * ops.mask[:, None], TOL["fp64"], (name, "Sinv variant 1"))
+        Xs = to_dev(X, "tf32", cfg.complex)
+        Ys = torch.empty_like(Xs)
+        ctx.apply_HSinv(TF32, Xs, Ys, B, B)
+        torch.cuda.synchronize()
+        check(to_host(Ys, cfg.complex), ops.apply_H(ops.apply_Sinv(to_host(Xs, cfg.complex))) * ops.mask[:, None], TOL["tf32"],
+              (name, "HSinv variant 1"))
+        b0, bW, bU = bounds(ops, lam)
+        want = chfsi.filter_residual(ops.apply_H, ops.apply_S, ops.apply_Sinv, X, lam, m, b0, bW, bU)
+        got = run_filter(ctx, "tf32", m, b0, bW, bU, to_dev(X, "tf32", cfg.complex), lam, B)
+        check(to_host(got, cfg.complex), want, FILTER_TOL["tf32"], (name, "filter variant 1"))
+        ctx.set_sinv_variant(0)
+        assert relerr(ctx.get_sinv_coupling(cfg.natoms, cfg.nproj), ops0.dSinv) < 1e-11
+    finally:
+        ctx.destroy()

@@ -228,3 +228,22 @@ def test_apply_HSinv_rows_equals_assembled_rows(name):
     # the W half matters: without the low-rank part of S^-1approx the rows differ at O(1e-2)
     plain = ops.apply_H(ops.md_inv[:, None] * X * ops.mask[:, None]) * ops.mask[:, None]
     assert max(np.abs(plain[J] - want[J]).max() for J, _ in got) > 1e-4 * scale
+
+
+def test_projector_overlap_matrix_is_the_gram_matrix():
+    """paw.projector_overlap_matrix (the <p_alpha|p_beta> of PAPER.md:L228, used by the S^-1approx variant 1) against a brute-force
+    3-D quadrature of the projector functions themselves (paw.projector_values on a Gauss-Legendre grid over the cutoff cube):
+    pins the (l, m) block structure, the radial integrals and the cross-channel entries of the 13-projector set."""
+    cfg = dataclasses.replace(get_config(0), nproj=13)
+    sysd = make_system(cfg)
+    O = paw.projector_overlap_matrix(sysd)
+    x, w = np.polynomial.legendre.leggauss(64)
+    g = sysd.rc * x
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    W = (sysd.rc ** 3) * (w[:, None, None] * w[None, :, None] * w[None, None, :]).reshape(-1)
+    P = paw.projector_values(sysd, np.stack([X.reshape(-1), Y.reshape(-1), Z.reshape(-1)], axis=1))
+    brute = (P * W) @ P.T
+    assert np.abs(O - brute).max() < 2e-3          # the C^1 cutoff on a tensor grid: quadrature error of the brute force
+    assert np.allclose(np.diag(O), 1.0, atol=1e-10)            # unit-norm projectors
+    assert abs(O[0, 1]) > 0.5 and O[0, 2] == 0.0               # s / s' channels overlap strongly; s and p do not
+    assert np.allclose(O, O.T)
