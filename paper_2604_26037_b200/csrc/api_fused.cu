@@ -32,6 +32,7 @@ struct FusedPlan {
   int Bcap = 0; long ldw = 0;
   float* d_P1 = nullptr;        // [natoms][npj][ldw]
   float* d_Ppart = nullptr;     // [npairs][npj][ldw] per-pair partial projections (summed in pair order by k_psum)
+  uint4* d_CdF = nullptr;       // [npairs][ceil(n/8)][32]: the pairs' blocks as mma.sync A fragments, rounded to TF32 (k_build_cdf)
   float* d_Wcat = nullptr;      // [natoms][32][ldw]: rows [0,npj) W, [npj,2npj) D P2, rest 0
   float* d_Wcat_lo = nullptr;   // low parts of Wcat (FP32 mode, 3xTF32 split)
   float* d_Bext_lo = nullptr;   // low parts of d_Bext (built on first FP32-mode use)
@@ -311,6 +312,145 @@ size_t proj_cell_smem(int n) {
   return ((size_t)n * kPcVT + proj_cell_cs_floats<NPJ, CPLX>(n)) * sizeof(float) + (size_t)n * sizeof(long);
 }
 
+// The pairs' blocks in the order mma.sync m16n8k8 wants its A fragments, rounded to TF32 (round to nearest), zero beyond the
+// npj projectors and the n nodes:  CdF[pair][ks][lane] = { C[g][8ks+t], C[g+8][8ks+t], C[g][8ks+t+4], C[g+8][8ks+t+4] },
+// g = lane >> 2, t = lane & 3, C[al][I] = Cd[pair][al][I].  Real contexts, built once per plan.
+__global__ void __launch_bounds__(256)
+k_build_cdf(long total, int npj, int n, int nks, const float* __restrict__ Cd, uint4* __restrict__ CdF) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+    const int lane = (int)(i & 31), g = lane >> 2, t = lane & 3;
+    const long sl = i >> 5;
+    const int ks = (int)(sl % nks);
+    const long pr = sl / nks;
+    auto val = [&](int row, int col) -> uint32_t {
+      return row < npj && col < n ? ptx::cvt_rna_tf32(Cd[(pr * npj + row) * n + col]) : 0u;
+    };
+    const int c0 = ks * 8 + t;
+    CdF[i] = make_uint4(val(g, c0), val(g + 8, c0), val(g, c0 + 4), val(g + 8, c0 + 4));
+  }
+}
+
+// The same projection on the tensor cores, for the TF32 mode of a real context: per pair P(16 x 64) += A(16 x 8) B(8 x 64) over
+// the 43 (p = 6) row slices of 8 nodes, warp w taking slices w, w + 8, ... (mma.sync m16n8k8, TF32 operands, FP32 accumulate:
+// the precision the cell kernel next to it multiplies in).  A = the pair's block, read straight from global memory one pair
+// ahead, as ready-made fragments (k_build_cdf: one coalesced 16-byte load per lane and slice, each used by one warp only); B = the cell's rows in shared
+// memory, 16-byte pieces XOR-swizzled by (row & 3) so that the four k rows of a fragment load fall on different banks.
+// The eight warps' partial tiles are summed in the fixed order of k_proj_cell (w + 4 onto w, then 0..3): bit-reproducible.
+constexpr int kPmRedLd = 72;   // floats per row of the reduction scratch (72 mod 32 = 8: the float2 stores of a tile do not collide)
+template <int NPJ, int MAXJ>   // MAXJ: row slices per warp, ceil(ceil(n / 8) / 8)
+__global__ void __launch_bounds__(256, 2)
+k_proj_cell_mma(MeshDev md, const int* __restrict__ pcells, const int* __restrict__ cps, const int* __restrict__ cpi,
+                const uint4* __restrict__ CdF, const float* __restrict__ X, long ldx, int Wr, float* __restrict__ Ppart, long ldp) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  static_assert(NPJ <= 16, "one m16 tile");
+  const int n = md.n, n1 = md.n1;
+  const int nks = (n + 7) / 8;
+  float* tile = reinterpret_cast<float*>(smem_raw);                         // [8 nks][64], swizzled; rows >= n are zero
+  float* red = tile + (size_t)nks * 8 * kPcVT;                              // [4][NPJ][72]
+  long* nodeO = reinterpret_cast<long*>(red + 4 * NPJ * kPmRedLd);          // [n]
+  const int e = pcells[blockIdx.x];
+  const int v0 = blockIdx.y * kPcVT;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+  uint32_t a[MAXJ][4];
+  // slice j of a pair's block: rows g, g + 8 (projector), columns 8 ks + t, + 4 (node)
+  auto load_a = [&](const uint4* Cp, int j) {                               // Cp: the pair's fragments + lane
+    const int ks = w + 8 * j;
+    const uint4 v = ks < nks ? __ldg(Cp + 32 * ks) : make_uint4(0u, 0u, 0u, 0u);
+    a[j][0] = v.x; a[j][1] = v.y; a[j][2] = v.z; a[j][3] = v.w;
+  };
+  const int q0 = cps[e], q1 = cps[e + 1];
+  {
+    const uint4* Cp = CdF + (long)cpi[q0] * nks * 32 + lane;
+#pragma unroll
+    for (int j = 0; j < MAXJ; ++j) load_a(Cp, j);
+  }
+  {
+    int cx, cy, cz;
+    mesh_cell_coords(md, e, &cx, &cy, &cz);
+    for (int I = threadIdx.x; I < n; I += 256) {
+      int c = I % n1, b = (I / n1) % n1, aa = I / (n1 * n1), ix, iy, iz;
+      const long J = mesh_node(md, cx, cy, cz, aa, b, c, &ix, &iy, &iz);
+      nodeO[I] = md.mdinv1[0][ix] * md.mdinv1[1][iy] * md.mdinv1[2][iz] != 0.0 ? J * ldx : -1;
+    }
+  }
+  __syncthreads();
+  const uint32_t tile_a = ptx::smem_u32(tile);
+  for (int i = threadIdx.x; i < nks * 8 * (kPcVT / 4); i += 256) {
+    const int I = i >> 4, q = i & 15;
+    const long off = I < n ? nodeO[I] : -1;
+    const bool ok = off >= 0 && v0 + 4 * q < Wr;
+    ptx::cp_async16(tile_a + (uint32_t)(I * kPcVT + 4 * (q ^ ((I & 3) << 1))) * 4, ok ? X + off + v0 + 4 * q : X, ok ? 16u : 0u);
+  }
+  ptx::cp_async_commit();
+  ptx::cp_async_wait<0>();
+  __syncthreads();
+  // byte address of (row 8 ks + t, logical column 8 nt + g) = rowb + o[nt & 3] + 128 (nt >> 2); row + 4: + 1024
+  const uint32_t o0 = (uint32_t)((((0 ^ t) << 3) + g) * 4), o1 = (uint32_t)((((1 ^ t) << 3) + g) * 4),
+                 o2 = (uint32_t)((((2 ^ t) << 3) + g) * 4), o3 = (uint32_t)((((3 ^ t) << 3) + g) * 4);
+  for (int q = q0; q < q1; ++q) {
+    const int pr = cpi[q];
+    const uint4* Cnext = q + 1 < q1 ? CdF + (long)cpi[q + 1] * nks * 32 + lane : nullptr;
+    float acc[8][4];
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+#pragma unroll
+    for (int j = 0; j < MAXJ; ++j) {
+      const int ks = w + 8 * j;
+      if (ks < nks) {                                                        // (warp-uniform)
+        const uint32_t rowb = tile_a + (uint32_t)((ks * 8 + t) * kPcVT) * 4;
+#define PM_MMA(NT, O)                                                                                             \
+        ptx::mma_m16n8k8_tf32(acc[NT], a[j], ptx::lds_u32_off<128 * ((NT) >> 2)>(rowb + (O)),                     \
+                              ptx::lds_u32_off<1024 + 128 * ((NT) >> 2)>(rowb + (O)));
+        PM_MMA(0, o0) PM_MMA(1, o1) PM_MMA(2, o2) PM_MMA(3, o3) PM_MMA(4, o0) PM_MMA(5, o1) PM_MMA(6, o2) PM_MMA(7, o3)
+#undef PM_MMA
+      }
+      if (Cnext) load_a(Cnext, j);                                           // the next pair's slice, in flight behind this pair's work
+    }
+    if (w >= 4) {
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        float* r0 = red + ((size_t)(w - 4) * NPJ + g) * kPmRedLd + nt * 8 + 2 * t;
+        if (g < NPJ) *reinterpret_cast<float2*>(r0) = make_float2(acc[nt][0], acc[nt][1]);
+        if (g + 8 < NPJ) *reinterpret_cast<float2*>(r0 + 8 * kPmRedLd) = make_float2(acc[nt][2], acc[nt][3]);
+      }
+    }
+    __syncthreads();
+    if (w < 4) {
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        float* r0 = red + ((size_t)w * NPJ + g) * kPmRedLd + nt * 8 + 2 * t;
+        float2 u;
+        if (g < NPJ) {
+          u = *reinterpret_cast<float2*>(r0);
+          *reinterpret_cast<float2*>(r0) = make_float2(acc[nt][0] + u.x, acc[nt][1] + u.y);
+        }
+        if (g + 8 < NPJ) {
+          u = *reinterpret_cast<float2*>(r0 + 8 * kPmRedLd);
+          *reinterpret_cast<float2*>(r0 + 8 * kPmRedLd) = make_float2(acc[nt][2] + u.x, acc[nt][3] + u.y);
+        }
+      }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NPJ * 16; i += 256) {
+      const int al = i >> 4, qq = i & 15;
+      if (v0 + 4 * qq < Wr) {
+        float4 s = *reinterpret_cast<const float4*>(&red[(size_t)al * kPmRedLd + 4 * qq]);
+#pragma unroll
+        for (int ww = 1; ww < 4; ++ww) {
+          const float4 u = *reinterpret_cast<const float4*>(&red[((size_t)ww * NPJ + al) * kPmRedLd + 4 * qq]);
+          s.x += u.x; s.y += u.y; s.z += u.z; s.w += u.w;
+        }
+        *reinterpret_cast<float4*>(Ppart + ((long)pr * NPJ + al) * ldp + v0 + 4 * qq) = s;
+      }
+    }
+    __syncthreads();   // red is free for the next pair
+  }
+}
+template <int NPJ>
+size_t proj_cell_mma_smem(int n) {
+  return ((size_t)((n + 7) / 8) * 8 * kPcVT + 4 * NPJ * kPmRedLd) * sizeof(float) + (size_t)n * sizeof(long);
+}
+
 // P[a][al][.] = sum over the atom's pairs, in pair order, of the per-pair partial projections (k_proj_cell):
 // the ordered replacement of their cross-CTA reductions.  grid = (natoms * npj, ceil(Wq / 128)), block = 128; Wq = quads
 // of 4 real columns that hold data; ldq = leading dimension / 4.
@@ -343,7 +483,7 @@ k_psum(int npj, const int* __restrict__ aps, const float4* __restrict__ Ppart, l
 //   Wcat[a][k][v]: k < npj -> W, npj <= k < 2 npj -> W2; columns B <= v < Bpad (the pad columns of a ragged block the cell
 //   kernel's 16-byte gathers touch) are written as 0.  grid = (natoms, ceil(Bpad/32)), block = 32 * npj: one thread per
 //   (output row al, vector), so the dependent chain per thread is one dot product per neighbour instead of npj of them;
-//   P2 goes through shared memory for the last product.
+//   P1 slices, G^{ab} Delta^b_Sinv and P2 go through shared memory.
 // ------------------------------------------------------------------------------------------------
 constexpr int kCoupleLanes = 32;
 template <typename T>   // float (real context) or float2 (complex context); ldp, ldw in units of T
@@ -351,36 +491,50 @@ __global__ void __launch_bounds__(kCoupleLanes * PAWFE_MAX_NPJ)
 k_couple(int npj, int mode, const T* __restrict__ P1, long ldp, int B, int Bpad, const T* __restrict__ dSinv,
          const T* __restrict__ D, const int* __restrict__ nb_start, const int* __restrict__ nb_atom,
          const T* __restrict__ GD, T* __restrict__ Wcat, long ldw) {
-  __shared__ T p2s[PAWFE_MAX_NPJ][kCoupleLanes + 1];
+  // every operand is staged once per CTA: thread (al, lane) fetches ONE element of an atom's npj x 32 slice of P1 and
+  // (tid < npj^2) one element of the neighbour's G^{ab} Delta^b_Sinv, one neighbour ahead of the products that read them
+  // from shared memory.  The order of the additions is the one of the definition above (be = 0 .. npj-1, neighbours in list order).
+  __shared__ T own[PAWFE_MAX_NPJ][kCoupleLanes];
+  __shared__ T p2s[PAWFE_MAX_NPJ][kCoupleLanes];
+  __shared__ T pbs[2][PAWFE_MAX_NPJ][kCoupleLanes];
+  __shared__ T gs[2][PAWFE_MAX_NPJ * PAWFE_MAX_NPJ];
   const int a = blockIdx.x;
-  const int lane = threadIdx.x % kCoupleLanes, al = threadIdx.x / kCoupleLanes;   // al < npj
-  const int v = blockIdx.y * kCoupleLanes + lane;
+  const int tid = threadIdx.x, lane = tid % kCoupleLanes, al = tid / kCoupleLanes;   // al < npj
+  const int v = blockIdx.y * kCoupleLanes + lane, nn = npj * npj;
   const bool ok = v < B, wr = v < Bpad;   // wr && !ok: pad column, every product below is zero
-  T p1[PAWFE_MAX_NPJ];
-#pragma unroll
-  for (int be = 0; be < PAWFE_MAX_NPJ; ++be) p1[be] = (ok && be < npj) ? P1[((long)a * npj + be) * ldp + v] : s_zero(T());
+  const int s0 = mode == 0 ? nb_start[a] : 0, s1 = mode == 0 ? nb_start[a + 1] : 0;
+  T pre = s_zero(T()), gpre = s_zero(T());
+  auto fetch = [&](int s) {
+    const int b = nb_atom[s];
+    pre = ok ? P1[((long)b * npj + al) * ldp + v] : s_zero(T());
+    if (tid < nn) gpre = GD[(long)s * nn + tid];
+  };
+  if (s0 < s1) fetch(s0);
+  T p2 = ok ? P1[((long)a * npj + al) * ldp + v] : s_zero(T());
+  own[al][lane] = p2;
+  __syncthreads();
   T* Wa = Wcat + (long)a * 32 * ldw;
   if (mode != 2) {
     const T* S = dSinv + ((long)a * npj + al) * npj;
     T s = s_zero(T());
 #pragma unroll
-    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[be], p1[be]);
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(s, S[be], own[be][lane]);
     if (wr) Wa[(long)al * ldw + v] = s;
   } else if (wr) {
     Wa[(long)al * ldw + v] = s_zero(T());
   }
   if (mode == 1) return;
-  T p2 = ok ? P1[((long)a * npj + al) * ldp + v] : s_zero(T());
-  if (mode == 0) {
-    for (int s = nb_start[a]; s < nb_start[a + 1]; ++s) {
-      const int b = nb_atom[s];
-      const T* g = GD + ((long)s * npj + al) * npj;
-      T t = s_zero(T());
+  for (int s = s0; s < s1; ++s) {
+    const int buf = (s - s0) & 1;
+    pbs[buf][al][lane] = pre;
+    if (tid < nn) gs[buf][tid] = gpre;
+    __syncthreads();   // (two buffers: the writes of neighbour s + 2 come after the barrier of s + 1, past every read of s)
+    if (s + 1 < s1) fetch(s + 1);
+    const T* g = &gs[buf][al * npj];
+    T t = s_zero(T());
 #pragma unroll
-      for (int be = 0; be < PAWFE_MAX_NPJ; ++be)
-        if (be < npj) s_fma(t, g[be], ok ? P1[((long)b * npj + be) * ldp + v] : s_zero(T()));
-      p2 = s_add(p2, s_scale(t, -1.0));
-    }
+    for (int be = 0; be < PAWFE_MAX_NPJ; ++be) if (be < npj) s_fma(t, g[be], pbs[buf][be][lane]);
+    p2 = s_add(p2, s_scale(t, -1.0));
   }
   p2s[al][lane] = p2;
   __syncthreads();
@@ -483,7 +637,7 @@ void free_plan(FusedPlan* p) {
   cudaFree(p->d_ext_start); cudaFree(p->d_ext_atom); cudaFree(p->d_Bext);
   cudaFree(p->d_nb_start); cudaFree(p->d_nb_atom); cudaFree(p->d_GD); cudaFree(p->d_cps); cudaFree(p->d_cpi); cudaFree(p->d_pcells);
   cudaFree(p->d_P1); cudaFree(p->d_Ppart); cudaFree(p->d_Wcat); cudaFree(p->d_P64); cudaFree(p->d_W64);
-  cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo);
+  cudaFree(p->d_Wcat_lo); cudaFree(p->d_Bext_lo); cudaFree(p->d_xlo); cudaFree(p->d_CdF);
   if (p->aux) cudaStreamDestroy(p->aux);
   if (p->ev_fork) cudaEventDestroy(p->ev_fork);
   if (p->ev_join) cudaEventDestroy(p->ev_join);
@@ -656,7 +810,21 @@ pawfe_status ensure_block(pawfe_ctx* c, FusedPlan* p, float** buf, size_t* have,
 
 // P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple).
 // X: the block as floats (complex: interleaved), ldx in floats; B vectors.
-pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long ldx, int B, int mode) {
+// the fragment-ordered TF32 copy of the projector blocks (real contexts, n <= 512): built on the first TF32 projection of a
+// plan, or ahead of the hot calls by pawfe_prepare(PAWFE_TF32, ..)
+bool proj_mma_usable(const pawfe_ctx* c, const FusedPlan* p) { return !c->cplx && c->n <= 512 && p->npcells > 0; }
+pawfe_status ensure_cdf(pawfe_ctx* c, FusedPlan* p) {
+  if (p->d_CdF || !proj_mma_usable(c, p)) return PAWFE_OK;
+  const int nks = (c->n + 7) / 8;
+  const long total = (long)c->npairs * nks * 32;
+  TRY(dev_alloc(c, &p->d_CdF, (size_t)total));
+  k_build_cdf<<<8 * c->sm_count, 256, 0, c->stream>>>(total, c->npj, c->n, nks, (const float*)c->d_Cd32, p->d_CdF);
+  KERNEL_CHECK(c, "k_build_cdf");
+  return PAWFE_OK;
+}
+
+// tf32: the caller multiplies in TF32 (PAWFE_TF32 mode): a real context then projects on the tensor cores (k_proj_cell_mma).
+pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, bool tf32, const float* X, long ldx, int B, int mode) {
   if (c->npairs == 0) return PAWFE_OK;
   const int n = c->n, npj = c->npj;
   // per-pair partial projections, then their sum in pair order (no cross-CTA reductions: bit-reproducible)
@@ -671,7 +839,28 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, const float* X, long
   // 1's pair-parallel k_proj2 / k_projF, which read a cell's rows once per pair (profiles/r02_projection_kernels.md: config 4
   // 7.65 -> 4.53 ms per step, configs 1 / 2 / 3: 0.29 / 3.15 / 1.76 -> 0.27 / 2.59 / 1.24 ms).
   const int Wr = B * (c->cplx ? 2 : 1);
-  if (p->npcells > 0) {
+  if (tf32 && proj_mma_usable(c, p)) {
+    TRY(ensure_cdf(c, p));
+    const dim3 grid((unsigned)p->npcells, ceil_div(Wr, kPcVT));
+#define LAUNCH_PM(N, J)                                                                                                     \
+    do {                                                                                                                    \
+      TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell_mma<N, J>, smem));                                                  \
+      k_proj_cell_mma<N, J><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, p->d_CdF, X, ldx, Wr,        \
+                                                            p->d_Ppart, p->ldw);                                            \
+    } while (0)
+#define CASE_PM(N)                                                                                                          \
+    case N: {                                                                                                               \
+      const size_t smem = proj_cell_mma_smem<N>(n);                                                                         \
+      if (n <= 384) LAUNCH_PM(N, 6); else LAUNCH_PM(N, 8);                                                                  \
+    } break;
+    switch (npj) {
+      CASE_PM(1) CASE_PM(2) CASE_PM(3) CASE_PM(4) CASE_PM(5) CASE_PM(6) CASE_PM(7) CASE_PM(8)
+      CASE_PM(9) CASE_PM(10) CASE_PM(11) CASE_PM(12) CASE_PM(13) CASE_PM(14) CASE_PM(15) CASE_PM(16)
+    }
+#undef LAUNCH_PM
+#undef CASE_PM
+    KERNEL_CHECK(c, "k_proj_cell_mma");
+  } else if (p->npcells > 0) {
     const dim3 grid((unsigned)p->npcells, ceil_div(Wr, kPcVT));
 #define LAUNCH_PC(N, CP)                                                                                                   \
     do {                                                                                                                    \
@@ -808,6 +997,7 @@ pawfe_status fused_prepare_all(pawfe_ctx* c, pawfe_prec prec, int B, bool with_b
     }
     if (with_block) TRY(ensure_block(c, p, &p->d_xlo, &p->xlo_elems, blk));
   }
+  if (prec == PAWFE_TF32) TRY(ensure_cdf(c, p));
   if (with_block) TRY(ensure_block(c, p, &p->d_xs, &p->xs_elems, blk));
   return PAWFE_OK;
 }
@@ -859,7 +1049,7 @@ pawfe_status fused_apply_H(pawfe_ctx* c, pawfe_prec prec, const float* X, long l
   FusedPlan* p = (FusedPlan*)c->fused;
   if (prec == PAWFE_FP32) TRY(ensure_block(c, p, &p->d_xlo, &p->xlo_elems, (size_t)c->M * ldx));
   const int Wr = B * (c->cplx ? 2 : 1);   // X, Y as float blocks: ldx, ldy in floats, Wr real columns
-  TRY(project_and_couple(c, p, X, ldx, B, 2));
+  TRY(project_and_couple(c, p, prec == PAWFE_TF32, X, ldx, B, 2));
   return cell_pass(c, p, prec, X, ldx, Y, ldy, Wr, 1.0f, 0, epi_plain(TC_EPI_STORE), p->d_xlo);
 }
 
@@ -876,7 +1066,7 @@ pawfe_status fused_apply_HSinv(pawfe_ctx* c, pawfe_prec prec, const float* X, lo
   if (lds != Wr) CUDA_TRY(c, cudaMemsetAsync(p->d_xs, 0, (size_t)c->M * lds * sizeof(float), c->stream));   // pad columns
   k_scale_mdinv_f4<<<8 * c->sm_count, 256, 0, c->stream>>>(c->md, (const float4*)X, ldx / 4, (float4*)p->d_xs, lds / 4, Wr / 4);
   KERNEL_CHECK(c, "k_scale_mdinv_f4");
-  TRY(project_and_couple(c, p, p->d_xs, lds, B, 0));
+  TRY(project_and_couple(c, p, prec == PAWFE_TF32, p->d_xs, lds, B, 0));
   return cell_pass(c, p, prec, p->d_xs, lds, Y, ldy, Wr, 1.0f, 0, epi_plain(TC_EPI_STORE), p->d_xlo);
 }
 
@@ -951,14 +1141,14 @@ pawfe_status fused_filter(pawfe_ctx* c, pawfe_prec prec, int m, const double* ds
   //      bracket  -a c Rt_Y - zeta zeta1 Rt_X [FP32] + Yt (a Lambda_Y) [FP64 add, L374]  plus their own share of
   //      a M_D^-1 H T, the other cells add theirs in cell order ----
   for (int th = 2; th <= m; ++th) {
-    TRY(project_and_couple(c, p, RY, ldw, B, 0));
+    TRY(project_and_couple(c, p, prec == PAWFE_TF32, RY, ldw, B, 0));
     TcEpi epi;
     epi.mode = TC_EPI_BRACKET; epi.Yt = Yt; epi.aLam = ds + (size_t)(th - 1) * B; epi.ac = (float)acs[th]; epi.zz1 = (float)zzs[th]; epi.cw = cw;
     TRY(cell_pass(c, p, prec, RY, ldw, RX, ldw, Wr, (float)as[th], 1, epi, XLO));
     std::swap(RX, RY);
   }
   // ---- step 5: Psi_f = S^-1approx R_Y + X Lambda_Y = Rt_Y - M_D^-1 C W + X Lambda_Y ----
-  TRY(project_and_couple(c, p, RY, ldw, B, 1));
+  TRY(project_and_couple(c, p, prec == PAWFE_TF32, RY, ldw, B, 1));
   {
     const bool vec = (ldx & 3) == 0 && (reinterpret_cast<uintptr_t>(X) & 15) == 0;
     const dim3 grid((unsigned)c->ncell, ceil_div(Wr, 128));

@@ -416,7 +416,8 @@ def test_sinv_projector_overlap_variant(name):
     try:
         ctx.set_sinv_variant(1)
         assert relerr(ctx.get_sinv_coupling(cfg.natoms, cfg.nproj), ops.dSinv) < 1e-9
-        assert relerr(ops.dSinv, ops0.dSinv) > 1e-3                                    # the variant is a different matrix
+        # a different matrix, but only by the GLL quadrature error of the Gram matrix (the two forms of Eq. 29 agree as h -> 0)
+        assert 1e-8 < relerr(ops.dSinv, ops0.dSinv) < 1e-2
         B, m = cfg.block, cfg.degree
         X, lam = ritz_block(ops, cfg, B, stream=95)
         Xd = to_dev(X, "fp64", cfg.complex)
