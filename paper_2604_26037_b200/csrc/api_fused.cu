@@ -313,31 +313,36 @@ size_t proj_cell_smem(int n) {
 }
 
 // The pairs' blocks in the order mma.sync m16n8k8 wants its A fragments, rounded to TF32 (round to nearest), zero beyond the
-// npj projectors and the n nodes:  CdF[pair][ks][lane] = { C[g][8ks+t], C[g+8][8ks+t], C[g][8ks+t+4], C[g+8][8ks+t+4] },
-// g = lane >> 2, t = lane & 3, C[al][I] = Cd[pair][al][I].  Real contexts, built once per plan.
+// npj projectors and the n nodes:  CdF[pair][ks][part][lane] = { C[g][8ks+t], C[g+8][8ks+t], C[g][8ks+t+4], C[g+8][8ks+t+4] },
+// g = lane >> 2, t = lane & 3, C[al][I] = Cd[pair][al][I]; complex contexts (cw = 2): part 0 = Re C, part 1 = Im C.
+// Built once per plan.
 __global__ void __launch_bounds__(256)
-k_build_cdf(long total, int npj, int n, int nks, const float* __restrict__ Cd, uint4* __restrict__ CdF) {
+k_build_cdf(long total, int npj, int n, int nks, int cw, const float* __restrict__ Cd, uint4* __restrict__ CdF) {
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
     const int lane = (int)(i & 31), g = lane >> 2, t = lane & 3;
-    const long sl = i >> 5;
+    long sl = i >> 5;
+    const int part = (int)(sl % cw);
+    sl /= cw;
     const int ks = (int)(sl % nks);
     const long pr = sl / nks;
     auto val = [&](int row, int col) -> uint32_t {
-      return row < npj && col < n ? ptx::cvt_rna_tf32(Cd[(pr * npj + row) * n + col]) : 0u;
+      return row < npj && col < n ? ptx::cvt_rna_tf32(Cd[((pr * npj + row) * n + col) * cw + part]) : 0u;
     };
     const int c0 = ks * 8 + t;
     CdF[i] = make_uint4(val(g, c0), val(g + 8, c0), val(g, c0 + 4), val(g + 8, c0 + 4));
   }
 }
 
-// The same projection on the tensor cores, for the TF32 mode of a real context: per pair P(16 x 64) += A(16 x 8) B(8 x 64) over
+// The same projection on the tensor cores, for the TF32 mode: per pair P(16 x 64) += A(16 x 8) B(8 x 64) over
 // the 43 (p = 6) row slices of 8 nodes, warp w taking slices w, w + 8, ... (mma.sync m16n8k8, TF32 operands, FP32 accumulate:
 // the precision the cell kernel next to it multiplies in).  A = the pair's block, read straight from global memory one pair
 // ahead, as ready-made fragments (k_build_cdf: one coalesced 16-byte load per lane and slice, each used by one warp only); B = the cell's rows in shared
 // memory, 16-byte pieces XOR-swizzled by (row & 3) so that the four k rows of a fragment load fall on different banks.
 // The eight warps' partial tiles are summed in the fixed order of k_proj_cell (w + 4 onto w, then 0..3): bit-reproducible.
 constexpr int kPmRedLd = 72;   // floats per row of the reduction scratch (72 mod 32 = 8: the float2 stores of a tile do not collide)
-template <int NPJ, int MAXJ>   // MAXJ: row slices per warp, ceil(ceil(n / 8) / 8)
+// CPLX (interleaved (re, im) columns): P = Cr X + Ci X' with X'[2v] = -X[2v+1], X'[2v+1] = X[2v], i.e. a second MMA per tile whose
+// B fragment is read from the neighbouring column (g ^ 1) with the sign of the even columns flipped.
+template <int NPJ, int MAXJ, bool CPLX>   // MAXJ: row slices per warp, ceil(ceil(n / 8) / 8)
 __global__ void __launch_bounds__(256, 2)
 k_proj_cell_mma(MeshDev md, const int* __restrict__ pcells, const int* __restrict__ cps, const int* __restrict__ cpi,
                 const uint4* __restrict__ CdF, const float* __restrict__ X, long ldx, int Wr, float* __restrict__ Ppart, long ldp) {
@@ -351,16 +356,21 @@ k_proj_cell_mma(MeshDev md, const int* __restrict__ pcells, const int* __restric
   const int e = pcells[blockIdx.x];
   const int v0 = blockIdx.y * kPcVT;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
-  uint32_t a[MAXJ][4];
-  // slice j of a pair's block: rows g, g + 8 (projector), columns 8 ks + t, + 4 (node)
+  constexpr int cw = CPLX ? 2 : 1;
+  uint32_t a[MAXJ][4], ai[CPLX ? MAXJ : 1][4];
+  // slice j of a pair's block: rows g, g + 8 (projector), columns 8 ks + t, + 4 (node); complex: Re then Im
   auto load_a = [&](const uint4* Cp, int j) {                               // Cp: the pair's fragments + lane
     const int ks = w + 8 * j;
-    const uint4 v = ks < nks ? __ldg(Cp + 32 * ks) : make_uint4(0u, 0u, 0u, 0u);
+    const uint4 v = ks < nks ? __ldg(Cp + 32 * cw * ks) : make_uint4(0u, 0u, 0u, 0u);
     a[j][0] = v.x; a[j][1] = v.y; a[j][2] = v.z; a[j][3] = v.w;
+    if (CPLX) {
+      const uint4 u = ks < nks ? __ldg(Cp + 32 * (cw * ks + 1)) : make_uint4(0u, 0u, 0u, 0u);
+      ai[j][0] = u.x; ai[j][1] = u.y; ai[j][2] = u.z; ai[j][3] = u.w;
+    }
   };
   const int q0 = cps[e], q1 = cps[e + 1];
   {
-    const uint4* Cp = CdF + (long)cpi[q0] * nks * 32 + lane;
+    const uint4* Cp = CdF + (long)cpi[q0] * nks * (32 * cw) + lane;
 #pragma unroll
     for (int j = 0; j < MAXJ; ++j) load_a(Cp, j);
   }
@@ -387,9 +397,10 @@ k_proj_cell_mma(MeshDev md, const int* __restrict__ pcells, const int* __restric
   // byte address of (row 8 ks + t, logical column 8 nt + g) = rowb + o[nt & 3] + 128 (nt >> 2); row + 4: + 1024
   const uint32_t o0 = (uint32_t)((((0 ^ t) << 3) + g) * 4), o1 = (uint32_t)((((1 ^ t) << 3) + g) * 4),
                  o2 = (uint32_t)((((2 ^ t) << 3) + g) * 4), o3 = (uint32_t)((((3 ^ t) << 3) + g) * 4);
+  const uint32_t sgn = (g & 1) ? 0u : 0x80000000u;                         // complex: column g ^ 1 (offset ^ 4), even columns negated
   for (int q = q0; q < q1; ++q) {
     const int pr = cpi[q];
-    const uint4* Cnext = q + 1 < q1 ? CdF + (long)cpi[q + 1] * nks * 32 + lane : nullptr;
+    const uint4* Cnext = q + 1 < q1 ? CdF + (long)cpi[q + 1] * nks * (32 * cw) + lane : nullptr;
     float acc[8][4];
 #pragma unroll
     for (int nt = 0; nt < 8; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
@@ -400,7 +411,10 @@ k_proj_cell_mma(MeshDev md, const int* __restrict__ pcells, const int* __restric
         const uint32_t rowb = tile_a + (uint32_t)((ks * 8 + t) * kPcVT) * 4;
 #define PM_MMA(NT, O)                                                                                             \
         ptx::mma_m16n8k8_tf32(acc[NT], a[j], ptx::lds_u32_off<128 * ((NT) >> 2)>(rowb + (O)),                     \
-                              ptx::lds_u32_off<1024 + 128 * ((NT) >> 2)>(rowb + (O)));
+                              ptx::lds_u32_off<1024 + 128 * ((NT) >> 2)>(rowb + (O)));                            \
+        if (CPLX)                                                                                                 \
+          ptx::mma_m16n8k8_tf32(acc[NT], ai[j], ptx::lds_u32_off<128 * ((NT) >> 2)>(rowb + ((O) ^ 4u)) ^ sgn,     \
+                                ptx::lds_u32_off<1024 + 128 * ((NT) >> 2)>(rowb + ((O) ^ 4u)) ^ sgn);
         PM_MMA(0, o0) PM_MMA(1, o1) PM_MMA(2, o2) PM_MMA(3, o3) PM_MMA(4, o0) PM_MMA(5, o1) PM_MMA(6, o2) PM_MMA(7, o3)
 #undef PM_MMA
       }
@@ -810,15 +824,16 @@ pawfe_status ensure_block(pawfe_ctx* c, FusedPlan* p, float** buf, size_t* have,
 
 // P1 = C^T X (X already in the scaled variables), then the couplings in `mode` (see k_couple).
 // X: the block as floats (complex: interleaved), ldx in floats; B vectors.
-// the fragment-ordered TF32 copy of the projector blocks (real contexts, n <= 512): built on the first TF32 projection of a
+// the fragment-ordered TF32 copy of the projector blocks (n <= 512): built on the first TF32 projection of a
 // plan, or ahead of the hot calls by pawfe_prepare(PAWFE_TF32, ..)
-bool proj_mma_usable(const pawfe_ctx* c, const FusedPlan* p) { return !c->cplx && c->n <= 512 && p->npcells > 0; }
+bool proj_mma_usable(const pawfe_ctx* c, const FusedPlan* p) { return c->n <= 512 && p->npcells > 0; }
 pawfe_status ensure_cdf(pawfe_ctx* c, FusedPlan* p) {
   if (p->d_CdF || !proj_mma_usable(c, p)) return PAWFE_OK;
   const int nks = (c->n + 7) / 8;
-  const long total = (long)c->npairs * nks * 32;
+  const int cw = c->cplx ? 2 : 1;
+  const long total = (long)c->npairs * nks * cw * 32;
   TRY(dev_alloc(c, &p->d_CdF, (size_t)total));
-  k_build_cdf<<<8 * c->sm_count, 256, 0, c->stream>>>(total, c->npj, c->n, nks, (const float*)c->d_Cd32, p->d_CdF);
+  k_build_cdf<<<8 * c->sm_count, 256, 0, c->stream>>>(total, c->npj, c->n, nks, cw, (const float*)c->d_Cd32, p->d_CdF);
   KERNEL_CHECK(c, "k_build_cdf");
   return PAWFE_OK;
 }
@@ -844,9 +859,15 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, bool tf32, const flo
     const dim3 grid((unsigned)p->npcells, ceil_div(Wr, kPcVT));
 #define LAUNCH_PM(N, J)                                                                                                     \
     do {                                                                                                                    \
-      TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell_mma<N, J>, smem));                                                  \
-      k_proj_cell_mma<N, J><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, p->d_CdF, X, ldx, Wr,        \
-                                                            p->d_Ppart, p->ldw);                                            \
+      if (c->cplx) {                                                                                                        \
+        TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell_mma<N, J, true>, smem));                                          \
+        k_proj_cell_mma<N, J, true><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, p->d_CdF, X, ldx,    \
+                                                                    Wr, p->d_Ppart, p->ldw);                                \
+      } else {                                                                                                              \
+        TRY(pawfe_ensure_smem(c, (const void*)k_proj_cell_mma<N, J, false>, smem));                                         \
+        k_proj_cell_mma<N, J, false><<<grid, 256, smem, c->stream>>>(c->md, p->d_pcells, p->d_cps, p->d_cpi, p->d_CdF, X, ldx,   \
+                                                                     Wr, p->d_Ppart, p->ldw);                               \
+      }                                                                                                                     \
     } while (0)
 #define CASE_PM(N)                                                                                                          \
     case N: {                                                                                                               \
