@@ -62,8 +62,8 @@ typedef enum {
  *         FP32 accumulation; ~1e-6 relative per product), real and complex contexts alike; blocks that do not meet the
  *         tensor-core path's alignment rules use FP32 FMAs.
  *   TF32: FP32 storage; operands of the cell contraction truncated to TF32 inside tcgen05 tensor
- *         cores, FP32 accumulation (~7e-4 relative per product).  In the fused filter step and pawfe_apply_HSinv of a real
- *         context the projection C^dagger X is a TF32 tensor-core product too (projector blocks rounded to nearest, FP32
+ *         cores, FP32 accumulation (~7e-4 relative per product).  In the fused filter step and pawfe_apply_HSinv the
+ *         projection C^dagger X is a TF32 tensor-core product too (projector blocks rounded to nearest, FP32
  *         accumulation).  Nothing else is TF32. */
 typedef enum { PAWFE_FP64 = 0, PAWFE_FP32 = 1, PAWFE_TF32 = 2 } pawfe_prec;
 typedef enum { PAWFE_PERIODIC = 0, PAWFE_DIRICHLET = 1 } pawfe_bc;
