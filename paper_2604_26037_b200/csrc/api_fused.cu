@@ -851,8 +851,8 @@ pawfe_status project_and_couple(pawfe_ctx* c, FusedPlan* p, bool tf32, const flo
     return PAWFE_OK;
   };
   // Cell-parallel projection into per-pair partials (every pair belongs to exactly one cell of the list).  It replaced round
-  // 1's pair-parallel k_proj2 / k_projF, which read a cell's rows once per pair (profiles/r02_projection_kernels.md: config 4
-  // 7.65 -> 4.53 ms per step, configs 1 / 2 / 3: 0.29 / 3.15 / 1.76 -> 0.27 / 2.59 / 1.24 ms).
+  // 1's pair-parallel kernels, which read a cell's rows once per pair (profiles/r02_projection_kernels.md, configs 1 / 2 / 3 / 4:
+  // 0.29 / 3.15 / 1.76 / 7.65 ms per step -> FP32 FMA 0.27 / 2.59 / 1.24 / 4.45 -> tensor cores 0.20 / 1.59 / 0.93 / 2.33).
   const int Wr = B * (c->cplx ? 2 : 1);
   if (tf32 && proj_mma_usable(c, p)) {
     TRY(ensure_cdf(c, p));
